@@ -1,0 +1,333 @@
+// ca_kernels.cuh -- per-stage kernels of one CA step over the whole batch (sm_100a).
+// Stage numbering follows DESIGN.md section 4: S-SEED, S0 irradiate, S1 diffusion-reaction,
+// S2 cell state, S3 division, S4 counts/fitness.
+#pragma once
+#include "ca_device.cuh"
+
+namespace ca {
+
+// ------------------------------------------------------------------ S-SEED --
+// [D S-SEED] BASELINE configs[0]: fields at constant boundary values, WALL layer, cluster at centre,
+// phases uniform from the seed.  One thread per site of the whole batch.
+__global__ void k_seed(KParams P, Lattice L, ca_init init)
+{
+    const long long gi = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gi >= P.n * P.batch) return;
+    const int b = (int)(gi / P.n);
+    const uint32_t i = (uint32_t)(gi - (long long)b * P.n);
+    const int x = i % P.nx, y = (i / P.nx) % P.ny, z = i / (P.nx * P.ny);
+    const bool wall = x == 0 || y == 0 || z == 0 || x == P.nx - 1 || y == P.ny - 1 || z == P.nz - 1;
+#pragma unroll
+    for (int s = 0; s < 3; ++s) { L.f[0][s][gi] = P.boundary[s]; L.f[1][s][gi] = P.boundary[s]; }
+    uint8_t st = wall ? CA_WALL : CA_EMPTY;
+    uint16_t ck = 0;
+    if (!wall) {
+        const int cx = init.cx >= 0 ? init.cx : P.nx / 2;
+        const int cy = init.cy >= 0 ? init.cy : P.ny / 2;
+        const int cz = init.cz >= 0 ? init.cz : P.nz / 2;
+        const int dx = x - cx, dy = y - cy, dz = z - cz;
+        const int d2 = dx * dx + dy * dy + dz * dz;
+        bool place;
+        if (init.kind == 0) place = (d2 == 0);
+        else if (init.kind == 1) place = (d2 <= 1);
+        else place = ((double)d2 <= (double)init.radius * (double)init.radius);
+        if (place) {
+            const uint32_t sid = init.shared_init ? 0u : P.sim_id_base + (uint32_t)b;
+            const int kind = 1 + (int)uniform_int(rnd(P, i, 0u, sid, P_INIT_PHASE), 4u);
+            ck = (uint16_t)(1 + (int)uniform_int(rnd(P, i, 0u, sid, P_INIT_CLOCK), (uint32_t)P.T[kind - 1]));
+            int m = decide_mode(P, P.boundary[0], P.boundary[1], P.boundary[2]);
+            if (m < 0) m = 3;
+            st = (uint8_t)(kind | (m << 3));
+        }
+    }
+    L.state[gi] = st;
+    L.clock[gi] = ck;
+    L.damage[gi] = 0;
+}
+
+// ---------------------------------------------------------------------- S0 --
+// [D S0] Irradiation: LQ with incomplete repair, phase- and oxygen-dependent [D G10].  Launched by
+// the host only on steps where some simulation has a fraction scheduled; each
+// simulation checks its own fire-step table.  fp64 arithmetic: this runs on <= ~100 of 432 000 steps.
+// grid = (chunks, batch)
+__global__ void k_irradiate(KParams P, Lattice L, int cur, const int *__restrict__ fire, const float *__restrict__ dose,
+                            const int *__restrict__ nfrac, int max_frac, const long long *__restrict__ d_step, int k)
+{
+    const int b = blockIdx.y;
+    const long long step = *d_step + k;
+    const int nf = nfrac[b];
+    const int *fb = fire + (size_t)b * max_frac;
+    const float *db = dose + (size_t)b * max_frac;
+    bool any = false;
+    for (int j = 0; j < nf; ++j) any |= (fb[j] == (int)step && db[j] > 0.0f);
+    if (!any) return;
+    const uint32_t sid = P.sim_id_base + (uint32_t)b;
+    const double m = (double)P.oer_m, K = (double)P.oer_K;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < P.n; i += (long long)gridDim.x * blockDim.x) {
+        const long long gi = (long long)b * P.n + i;
+        uint32_t st = L.state[gi];
+        if (!is_live(st)) continue;
+        const int kind = st & 7;
+        const double O = (double)L.f[cur][0][gi];
+        const double omf = (m * O + K) / ((O + K) * m);
+        const double al = (double)P.alpha[kind - 1], be = (double)P.beta[kind - 1];
+        uint32_t D = L.damage[gi];
+        for (int j = 0; j < nf; ++j) {
+            if (fb[j] != (int)step) continue;
+            const double d = (double)db[j];
+            if (!(d > 0.0)) continue;
+            const double de = d * omf;
+            const double Dg = (double)D / 1024.0;
+            const double E = al * de + be * de * de + 2.0 * be * de * Dg;
+            const double pk = -expm1(-E);
+            double t = floor(pk * 4294967296.0);                      // [D G23]
+            const uint32_t T = t >= 4294967295.0 ? 4294967295u : (t <= 0.0 ? 0u : (uint32_t)t);
+            if (rnd(P, (uint32_t)i, (uint32_t)step, sid, P_IRRADIATE, (uint32_t)j) < T) st |= CA_DOOMED;
+            const double nd = (double)D + floor(1024.0 * de + 0.5);  // [D G24]
+            D = nd > 65535.0 ? 65535u : (uint32_t)nd;
+        }
+        L.state[gi] = (uint8_t)st;
+        L.damage[gi] = (uint16_t)D;
+    }
+}
+
+// ---------------------------------------------------------------------- S1 --
+// [D S1] ONE explicit 7-point Jacobi sub-step of all three species, plain global loads.
+// Reference-grade kernel (the `fused = 0` path): one launch per sub-step, 25 B/site of traffic each.
+__global__ void k_diffuse_sub(KParams P, Lattice L, int src)
+{
+    const long long gi = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gi >= P.n * P.batch) return;
+    const uint32_t i = (uint32_t)(gi % P.n);
+    const int x = i % P.nx, y = (i / P.nx) % P.ny, z = i / (P.nx * P.ny);
+    const bool wall = x == 0 || y == 0 || z == 0 || x == P.nx - 1 || y == P.ny - 1 || z == P.nz - 1;
+    const int dst = src ^ 1;
+    if (wall) {
+#pragma unroll
+        for (int s = 0; s < 3; ++s) L.f[dst][s][gi] = L.f[src][s][gi];
+        return;
+    }
+    const uint32_t st = L.state[gi];
+    const bool lv = is_live(st);
+    const int mode = (st >> 3) & 3;
+    const long long sy = P.nx, sz = (long long)P.nx * P.ny;
+#pragma unroll
+    for (int s = 0; s < 3; ++s) {
+        const float *a = L.f[src][s];
+        const float r = lv ? P.rate[s][mode] : 0.0f;
+        L.f[dst][s][gi] = stencil_point(a[gi], a[gi - 1], a[gi + 1], a[gi - sy], a[gi + sy], a[gi - sz], a[gi + sz],
+                                        P.lambda[s], r);
+    }
+}
+
+// ---------------------------------------------------------------------- S2 --
+// [D S2] Per-site cell-state update, in place (a site reads only itself and the post-S1 fields).
+__device__ __forceinline__ void cell_update(const KParams &P, uint32_t &st, uint32_t &ck, uint32_t &dm,
+                                            float O, float G, float H, uint32_t site, uint32_t step, uint32_t sid)
+{
+    const int kind = st & 7;
+    if (kind == CA_DEAD) {
+        ck -= 1;
+        if (ck == 0) { st = CA_EMPTY; dm = 0; }
+        return;
+    }
+    const int mode = decide_mode(P, O, G, H);                            // (i) metabolism [D G5]
+    if (mode < 0) { st = CA_DEAD; ck = (uint32_t)P.lysis_steps; dm = 0; return; }
+    st = (st & ~0x18u) | ((uint32_t)mode << 3);
+    if (dm > 0 && (step + 1) % (uint32_t)P.repair_period == 0) {          // (ii) repair [D G11]
+        uint32_t dec = dm >> P.repair_shift;
+        dm -= dec < 1 ? 1 : dec;
+    }
+    if (mode < 2 && !(st & CA_READY)) {                                    // (iii) cycle [D G6, G7]
+        ck -= 1;
+        if (ck == 0) {
+            if (kind == CA_G1 || kind == CA_S) {
+                st = (st & ~7u) | (uint32_t)(kind + 1);
+                ck = draw_clock(P, kind + 1, site, step, sid, P_PHASE_CLOCK);
+            } else if (kind == CA_G2) {
+                if (st & CA_DOOMED) { st = CA_DEAD; ck = (uint32_t)P.lysis_steps; dm = 0; return; }   // mitotic death [D G10]
+                st = (st & ~7u) | CA_M;
+                ck = draw_clock(P, CA_M, site, step, sid, P_PHASE_CLOCK);
+            } else {
+                st |= CA_READY;                                            // M finished: waits for space
+            }
+        }
+    }
+}
+
+__global__ void k_cells(KParams P, Lattice L, int cur, const long long *__restrict__ d_step, int k)
+{
+    const long long gi = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gi >= P.n * P.batch) return;
+    uint32_t st = L.state[gi];
+    const int kind = st & 7;
+    if (kind == CA_EMPTY || kind == CA_WALL) return;
+    const int b = (int)(gi / P.n);
+    const uint32_t i = (uint32_t)(gi - (long long)b * P.n);
+    const uint32_t step = (uint32_t)(*d_step + k);
+    uint32_t ck = L.clock[gi], dm = L.damage[gi];
+    const uint32_t st0 = st, ck0 = ck, dm0 = dm;
+    cell_update(P, st, ck, dm, L.f[cur][0][gi], L.f[cur][1][gi], L.f[cur][2][gi], i, step, P.sim_id_base + (uint32_t)b);
+    if (st != st0) L.state[gi] = (uint8_t)st;
+    if (ck != ck0) L.clock[gi] = (uint16_t)ck;
+    if (dm != dm0) L.damage[gi] = (uint16_t)dm;
+}
+
+// ---------------------------------------------------------------------- S3 --
+// [D S3, G8, G9] Division and placement with deterministic conflict resolution and no racy atomics:
+// every decision is a pure function of the post-S2 lattice, so the detect kernel only READS the
+// lattice and appends the winners (parent, direction) to a list; the apply kernel then writes them.
+//
+// choose_dir: the EMPTY face-neighbour of parent p with the smallest (Philox DIR key, dir); -1 if none.
+__device__ __forceinline__ int choose_dir(const KParams &P, const uint8_t *__restrict__ sb, uint32_t p,
+                                          uint32_t step, uint32_t sid, const int off[6])
+{
+    int best = -1;
+    uint32_t bk = 0;
+#pragma unroll
+    for (int d = 0; d < 6; ++d) {
+        if (sb[(int)p + off[d]] != CA_EMPTY) continue;                     // WALL != EMPTY: targets are interior
+        const uint32_t kk = rnd(P, p, step, sid, P_DIR, (uint32_t)d);
+        if (best < 0 || kk < bk) { best = d; bk = kk; }                    // ties -> lower dir
+    }
+    return best;
+}
+
+__global__ void k_div_detect(KParams P, Lattice L, const long long *__restrict__ d_step, int k,
+                             unsigned long long *__restrict__ winners, unsigned int *__restrict__ nwin,
+                             unsigned int cap, int *__restrict__ err)
+{
+    const long long gi = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gi >= P.n * P.batch) return;
+    if (!is_parent(L.state[gi])) return;
+    const int b = (int)(gi / P.n);
+    const uint32_t p = (uint32_t)(gi - (long long)b * P.n);
+    const uint8_t *sb = L.state + (long long)b * P.n;
+    const uint32_t step = (uint32_t)(*d_step + k);
+    const uint32_t sid = P.sim_id_base + (uint32_t)b;
+    const int off[6] = { -1, 1, -P.nx, P.nx, -P.nx * P.ny, P.nx * P.ny };
+    const int dir = choose_dir(P, sb, p, step, sid, off);
+    if (dir < 0) return;                                                   // blocked: stays READY, retries
+    const uint32_t e = (uint32_t)((int)p + off[dir]);
+    const uint32_t mykey = rnd(P, p, step, sid, P_CLAIM);
+#pragma unroll 1
+    for (int d = 0; d < 6; ++d) {                                          // competitors = other neighbours of e
+        const uint32_t q = (uint32_t)((int)e + off[d]);
+        if (q == p || !is_parent(sb[q])) continue;
+        const int dq = choose_dir(P, sb, q, step, sid, off);
+        if (dq < 0 || (uint32_t)((int)q + off[dq]) != e) continue;
+        const uint32_t qk = rnd(P, q, step, sid, P_CLAIM);
+        if (qk < mykey || (qk == mykey && q < p)) return;                  // lost: untouched, retries next step
+    }
+    const unsigned int slot = atomicAdd(nwin, 1u);                         // list order is irrelevant to the result
+    if (slot >= cap) { *err = CA_EOVERFLOW; return; }
+    winners[slot] = ((unsigned long long)gi << 3) | (unsigned long long)dir;
+}
+
+__global__ void k_div_apply(KParams P, Lattice L, const long long *__restrict__ d_step, int k,
+                            const unsigned long long *__restrict__ winners, const unsigned int *__restrict__ nwin,
+                            unsigned int cap)
+{
+    unsigned int n = *nwin;
+    if (n > cap) n = cap;
+    const uint32_t step = (uint32_t)(*d_step + k);
+    const int off[6] = { -1, 1, -P.nx, P.nx, -P.nx * P.ny, P.nx * P.ny };
+    for (unsigned int w = blockIdx.x * blockDim.x + threadIdx.x; w < n; w += gridDim.x * blockDim.x) {
+        const unsigned long long ent = winners[w];
+        const long long gp = (long long)(ent >> 3);
+        const int dir = (int)(ent & 7ull);
+        const int b = (int)(gp / P.n);
+        const uint32_t p = (uint32_t)(gp - (long long)b * P.n);
+        const uint32_t e = (uint32_t)((int)p + off[dir]);
+        const long long ge = gp + off[dir];
+        const uint32_t sid = P.sim_id_base + (uint32_t)b;
+        const uint32_t keep = L.state[gp] & (0x18u | CA_DOOMED);          // mode and DOOMED carried to both [D G10]
+        L.state[gp] = (uint8_t)(CA_G1 | keep);
+        L.clock[gp] = draw_clock(P, CA_G1, p, step, sid, P_PARENT_CLOCK);
+        L.state[ge] = (uint8_t)(CA_G1 | keep);
+        L.clock[ge] = draw_clock(P, CA_G1, e, step, sid, P_DAUGHTER_CLOCK);
+        L.damage[ge] = L.damage[gp];
+    }
+}
+
+// end of a group of `adv` steps: advance the device step counter, clear the per-step winner counters
+__global__ void k_advance(long long *d_step, int adv, unsigned int *nwin, int nslots)
+{
+    if (threadIdx.x == 0) *d_step += adv;
+    for (int i = threadIdx.x; i < nslots; i += blockDim.x) nwin[i] = 0;
+}
+
+// ---------------------------------------------------------------------- S4 --
+// [D S4] per-simulation counts by warp-shuffle reduction; grid = (blocks_per_sim, batch).
+// Each thread scans 16 state bytes per load; counts go to counts[b][CA_NCOUNT] by one atomic per warp.
+__global__ void k_counts(KParams P, const uint8_t *__restrict__ state, int *__restrict__ counts)
+{
+    const int b = blockIdx.y;
+    const uint8_t *sb = state + (long long)b * P.n;
+    int c[12];
+#pragma unroll
+    for (int q = 0; q < 12; ++q) c[q] = 0;
+    auto tally = [&](uint32_t st) {
+        const uint32_t kind = st & 7u;
+        const bool lv = kind >= 1u && kind <= 4u;
+        c[CA_C_LIVE] += lv;
+        c[CA_C_DOOMED] += lv && (st & CA_DOOMED);
+        c[CA_C_READY] += lv && (st & CA_READY);
+        c[CA_C_DEAD] += kind == CA_DEAD;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            c[CA_C_G1 + q] += kind == (uint32_t)(1 + q);
+            c[CA_C_PA + q] += lv && (((st >> 3) & 3u) == (uint32_t)q);
+        }
+    };
+    const long long nvec = ((long long)b * P.n % 16 == 0) ? P.n / 16 : 0;   // vector body only when 16B-aligned
+    const uint4 *sv = reinterpret_cast<const uint4 *>(sb);
+    for (long long v = (long long)blockIdx.x * blockDim.x + threadIdx.x; v < nvec; v += (long long)gridDim.x * blockDim.x) {
+        const uint4 w = sv[v];
+        const uint32_t ws[4] = { w.x, w.y, w.z, w.w };
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            if (ws[q] == 0u || ws[q] == 0x07070707u) continue;              // all EMPTY / all WALL
+#pragma unroll
+            for (int r = 0; r < 4; ++r) tally((ws[q] >> (8 * r)) & 0xFFu);
+        }
+    }
+    for (long long i = nvec * 16 + (long long)blockIdx.x * blockDim.x + threadIdx.x; i < P.n; i += (long long)gridDim.x * blockDim.x)
+        tally(sb[i]);
+#pragma unroll
+    for (int q = 0; q < 12; ++q) {
+        int v = c[q];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
+        if ((threadIdx.x & 31) == 0 && v) atomicAdd(&counts[b * CA_NCOUNT + q], v);   // integer: order-independent
+    }
+}
+
+// occupied = live + dead [D G13]; fitness = N_ref - occupied (Eq. 1)
+__global__ void k_finish_counts(KParams P, int *__restrict__ counts, float *__restrict__ fitness)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= P.batch) return;
+    const int occ = counts[b * CA_NCOUNT + CA_C_LIVE] + counts[b * CA_NCOUNT + CA_C_DEAD];
+    counts[b * CA_NCOUNT + CA_C_OCCUPIED] = occ;
+    const long long nref = P.N_ref > 0 ? (long long)P.N_ref : (long long)(P.nx - 2) * (P.ny - 2) * (P.nz - 2);
+    fitness[b] = (float)(nref - occ);
+}
+
+// broadcast simulation `src` to simulations [first, first+count) (skipping src itself); bytes per sim = nbytes (16B multiple not required)
+__global__ void k_broadcast(uint8_t *base, long long nbytes, int src, int first, int count)
+{
+    const int b = first + blockIdx.y;
+    if (b == src) return;
+    const uint8_t *s = base + (long long)src * nbytes;
+    uint8_t *d = base + (long long)b * nbytes;
+    if (nbytes % 16 == 0) {
+        const uint4 *sv = reinterpret_cast<const uint4 *>(s);
+        uint4 *dv = reinterpret_cast<uint4 *>(d);
+        for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nbytes / 16; i += (long long)gridDim.x * blockDim.x) dv[i] = sv[i];
+    } else {
+        for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nbytes; i += (long long)gridDim.x * blockDim.x) d[i] = s[i];
+    }
+}
+
+}  // namespace ca

@@ -1,0 +1,54 @@
+"""Comparison helpers for GPU <-> oracle parity (tests only)."""
+import numpy as np
+
+from oracle import ca_oracle as o
+
+FIELDS = ("o2", "glc", "h")
+
+
+def oracle_from_snapshot(snap, params, dims, rng_seed, sim_id, precision="f64"):
+    nx, ny, nz = dims
+    s = o.OracleSim(nx, ny, nz, params, precision=precision)
+    s.set_state(state=snap["state"], clock=snap["clock"], damage=snap["damage"],
+                o2=snap["o2"].astype(np.float64), glc=snap["glc"].astype(np.float64), h=snap["h"].astype(np.float64),
+                step=snap["step"])
+    s.set_rng(rng_seed, sim_id)
+    return s
+
+
+def assert_ints_equal(g, r, where=""):
+    for k in ("state", "clock", "damage"):
+        if not np.array_equal(g[k], r[k]):
+            bad = np.argwhere(g[k] != r[k])
+            z, y, x = bad[0]
+            raise AssertionError("%s: %s differs at %d sites, first (z,y,x)=(%d,%d,%d): gpu %d oracle %d"
+                                 % (where, k, len(bad), z, y, x, g[k][z, y, x], r[k][z, y, x]))
+    assert g["step"] == r["step"], (where, g["step"], r["step"])
+
+
+def field_rel_err(g, r, params):
+    """max over sites of |gpu - oracle| / max(|oracle|, 1e-3 * boundary)  (SURVEY 8(c) comparison protocol)"""
+    out = {}
+    for s, k in enumerate(FIELDS):
+        floor = 1e-3 * float(np.float32(params["boundary"][s]))
+        a = g[k].astype(np.float64)
+        b = r[k].astype(np.float64)
+        out[k] = float((np.abs(a - b) / np.maximum(np.abs(b), floor)).max())
+    return out
+
+
+def assert_fields_close(g, r, params, tol=1e-4, where=""):
+    err = field_rel_err(g, r, params)
+    for k, v in err.items():
+        assert v <= tol, "%s: field %s rel err %.3e > %.1e" % (where, k, v, tol)
+
+
+def assert_fields_bitwise(g, r32, where=""):
+    """r32 comes from the fp32 diagnostic build of the oracle (fields exported as double, exactly fp32 values)"""
+    for k in FIELDS:
+        a = g[k].view(np.uint32)
+        b = r32[k].astype(np.float32).view(np.uint32)
+        # +0 / -0 are the same value; compare values
+        if not np.array_equal(g[k], r32[k].astype(np.float32)):
+            bad = np.argwhere(g[k] != r32[k].astype(np.float32))
+            raise AssertionError("%s: field %s differs bitwise at %d sites, first %s" % (where, k, len(bad), bad[0]))

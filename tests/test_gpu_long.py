@@ -1,0 +1,80 @@
+"""Long-horizon and full-size parity: BASELINE configs[0] run whole; configs[1] in the launch
+configuration bench.py times, compared on snapshot windows the oracle can afford."""
+import numpy as np
+import pytest
+
+from oracle import ca_oracle as o
+from paper_2303_08123_b200 import binding, workloads as w
+from tests._parity import oracle_from_snapshot, assert_ints_equal, assert_fields_close, assert_fields_bitwise
+
+pytestmark = pytest.mark.gpu
+
+
+def test_c1_whole_run_final_counts():
+    """configs[0]: 32^3, 48 h, one 2 Gy fraction at 24 h.  Final counts within 1 % of the fp64 oracle
+    (north_star); the fp32 diagnostic oracle must agree bitwise at the end of the whole run."""
+    cfg = w.config(1)
+    p = w.default_params()
+    g = binding.CaBatch(1, *cfg["dims"], p)
+    g.seed(rng_seed=cfg["rng_seed"], **cfg["init"])
+    g.set_protocols(cfg["dose"], cfg["delay"], cfg["nfrac"], t0_h=cfg["t0_h"])
+    g.run(cfg["horizon_h"])
+    gs = g.get_state()
+    gc = g.counts()[0]
+    refs = {}
+    for prec in ("f64", "f32"):
+        r = o.OracleSim(*cfg["dims"], p, precision=prec)
+        r.seed(cfg["init"]["kind"], center=cfg["init"]["center"], rng_seed=cfg["rng_seed"], sim_id=0)
+        r.set_protocol(cfg["dose"][0], cfg["delay"][0], t0_h=cfg["t0_h"])
+        r.run(cfg["horizon_h"])
+        refs[prec] = r
+    assert gs["step"] == 28800
+    assert_ints_equal(gs, refs["f32"].get_state(), "c1 end, f32 oracle")
+    assert_fields_bitwise(gs, refs["f32"].get_state(), "c1 end, f32 oracle")
+    rc = refs["f64"].counts()
+    assert gc[0] > 7 and gc[3] > 0                          # it grew, and cells doomed by the fraction at 24 h died
+    for k in (0, 12):
+        assert abs(int(gc[k]) - int(rc[k])) <= max(1, 0.01 * rc[k]), (k, gc.tolist(), rc.tolist())
+    assert_fields_close(gs, refs["f64"].get_state(), p, 1e-4, "c1 end")
+    assert g.fitness()[0] == float(30 ** 3 - gc[12])
+    g.close()
+
+
+def test_c2_full_size_snapshot_windows():
+    """configs[1] at full size (64 sims x 64^3, the configuration bench.py times): run to checkpoints
+    (quasi-steady warm-up; just after the first fraction), export sampled simulations, let the oracle
+    advance each snapshot 50 steps, compare (SURVEY 8(c) comparison protocol (2))."""
+    cfg = w.config(2)
+    p = w.default_params()
+    dims = cfg["dims"]
+    g = binding.CaBatch(cfg["batch"], *dims, p, max_frac=10)
+    g.seed(rng_seed=cfg["rng_seed"], sim_id_base=cfg["sim_id_base"], **cfg["init"])
+    g.set_protocols(cfg["dose"], cfg["delay"], cfg["nfrac"], t0_h=cfg["t0_h"])
+    first_fire = int(round((cfg["t0_h"] + cfg["delay"][:, 0].min()) * 600))
+    b_first = int(np.argmin(cfg["delay"][:, 0]))
+    for checkpoint, sims in ((600, (0, 63)), (first_fire - 20, (b_first, 17))):
+        g.step(checkpoint - g.step_index)
+        snaps = {b: g.get_state(b) for b in sims}
+        g.step(50)
+        for b in sims:
+            after = g.get_state(b)
+            for prec in ("f64", "f32"):
+                r = oracle_from_snapshot(snaps[b], p, dims, cfg["rng_seed"], cfg["sim_id_base"] + b, prec)
+                nf = int(cfg["nfrac"][b])
+                # remaining fractions of this simulation, re-expressed from the snapshot's step
+                t = cfg["t0_h"] + np.cumsum(cfg["delay"][b, :nf])
+                keep = t * 600 >= snaps[b]["step"] - 1e-6
+                if keep.any():
+                    d = cfg["dose"][b, :nf][keep]
+                    tt = t[keep]
+                    r.set_protocol(d, np.diff(np.concatenate([[0.0], tt])), t0_h=0.0)
+                r.step(50)
+                ref = r.get_state()
+                assert_ints_equal(after, ref, "c2 sim %d @%d %s" % (b, checkpoint, prec))
+                if prec == "f32":
+                    assert_fields_bitwise(after, ref, "c2 sim %d @%d" % (b, checkpoint))
+                else:
+                    assert_fields_close(after, ref, p, 1e-4, "c2 sim %d @%d" % (b, checkpoint))
+    st = g.get_state(b_first)
+    assert (st["damage"] > 0).any()                          # the first fraction fired inside the second window
+    g.close()
