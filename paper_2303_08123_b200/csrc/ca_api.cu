@@ -79,6 +79,7 @@ struct ca_ctx {
     // options
     int graph_steps;
     int fused;
+    FusedPlan fplan;
     cudaGraphExec_t graph[2];      // indexed by the ping-pong parity at graph start
     int graph_len[2];
     long long graph_nodes;
@@ -115,10 +116,11 @@ int enqueue_step(ca_ctx *c, int cur, int k)
 {
     const KParams &P = c->P;
     const long long tot = P.n * P.batch;
-    if (c->fused && fused_supported(P)) {
-        launch_fused(P, c->L, cur, c->d_step, k, c->stream);               // S1 (all sub-steps) in one kernel
-        cur ^= 1;
-        c->launches += 1;
+    if (c->fused && fused_supported(c->fplan)) {
+        cudaError_t fe;
+        const int np = launch_fused(c->fplan, c->L, cur, c->stream, &fe);   // S1: all n_sub sub-steps, one pass over HBM (two if n_sub > 4)
+        if (np & 1) cur ^= 1;
+        c->launches += np;
     } else {
         for (int m = 0; m < P.n_sub; ++m) {                                // S1, one launch per sub-step
             k_diffuse_sub<<<blocks_for(tot, 256), 256, 0, c->stream>>>(P, c->L, cur);
@@ -318,7 +320,7 @@ int ca_create(ca_ctx **out, int batch, int nx, int ny, int nz, const ca_params *
     // zero the small control blocks (protocol tables, counters)
     e = cudaMemsetAsync(c->ws + c->Y.winners, 0, c->Y.total - c->Y.winners, c->stream);
     if (e != cudaSuccess) { int rc = cuda_fail(nullptr, e, "cudaMemsetAsync"); delete c; return rc; }
-    fused_configure(P);
+    fused_configure(P, c->fplan);
     *out = c;
     return CA_OK;
 }
@@ -513,7 +515,12 @@ int ca_stage(ca_ctx *c, int stage, int arg)
     switch (stage) {
     case 0: enqueue_irradiate(c); break;
     case 1:
-        if (c->fused && fused_supported(P)) { launch_fused(P, c->L, c->cur, c->d_step, 0, c->stream); c->cur ^= 1; c->launches += 1; }
+        if (c->fused && fused_supported(c->fplan)) {
+            cudaError_t fe;
+            const int np = launch_fused(c->fplan, c->L, c->cur, c->stream, &fe);
+            if (np & 1) c->cur ^= 1;
+            c->launches += np;
+        }
         else for (int m = 0; m < P.n_sub; ++m) { k_diffuse_sub<<<blocks_for(tot, 256), 256, 0, c->stream>>>(P, c->L, c->cur); c->cur ^= 1; c->launches += 1; }
         break;
     case 2: k_cells<<<blocks_for(tot, 256), 256, 0, c->stream>>>(P, c->L, c->cur, c->d_step, 0); c->launches += 1; break;

@@ -1,10 +1,426 @@
-// ca_fused.cuh -- temporally fused reaction-diffusion kernel (all n_sub sub-steps of S1 in one pass).
-// Placeholder interface for the first bring-up: reports "unsupported", so the per-sub-step kernel runs.
+// ca_fused.cuh -- temporally fused reaction-diffusion kernel: NL (<= 4) sub-steps of [D S1] in ONE pass over HBM.
+//
+// Why it looks like this: per site and CA step the stencil costs 12 x (8..9) fp32
+// operations against 25 bytes, so on B200 the FMA pipe (128 lanes/clk/SM) is as tight as HBM.  The kernel
+// therefore (a) reads and writes every field value once per CA step, (b) issues the arithmetic as packed
+// f32x2 instructions (same IEEE results as scalar add/mul/fma.rn, half the issue slots), and (c) keeps the
+// z-neighbours and all NL time levels of a lane's points in registers:
+//
+//   * a work unit is (simulation, species, range of z-planes); a persistent grid of one CTA per SM splits
+//     the flattened plane space evenly, so the only redundant work is the NL-deep cone at cuts inside a unit;
+//   * a CTA covers whole xy-planes (nx, ny <= 64, so no xy halo: the WALL layer closes the plane) and marches
+//     along z; a lane owns 2 (x) x 4 (y) points of the plane, a warp a 64 x 4 strip (two 32 x 4 strips
+//     when nx <= 32);
+//   * input planes and state planes arrive by bulk async copy (TMA 1-D, UBLKCP) into shared-memory rings,
+//     completion on mbarriers, 3 planes ahead;
+//   * level k (sub-step k) computes plane t-k while level 0 loads plane t: each level keeps 3 planes of its
+//     input level in registers (ring of 3, the march loop is unrolled by 3 so that no register is moved);
+//   * x-neighbours come from the neighbouring lane by shuffle, y-neighbours across strips through a small
+//     double-buffered shared-memory row exchange (one __syncthreads per plane);
+//   * the reaction term exists only where cells live (a few % of the lattice at configs[1]): each warp votes per
+//     plane on "any cell in my strip" and takes the path without source term and clamp when there is none
+//     (bit-identical there: v + 0 = v, and v >= 0 is guaranteed when 6*lambda*(1+2^-23) <= 1).
+//
+// Arithmetic per point is exactly [D S1]: sum6 = ((xm+xp)+(ym+yp))+(zm+zp); lap = sum6 - 6*c (product rounded
+// on its own); v = fma(lambda, lap, c); v += r; max(v, 0).  WALL points use lambda = 0, r = 0, which
+// returns c unchanged.
 #pragma once
 #include "ca_device.cuh"
 
 namespace ca {
-inline void fused_configure(const KParams &) {}
-inline bool fused_supported(const KParams &) { return false; }
-inline void launch_fused(const KParams &, const Lattice &, int, const long long *, int, cudaStream_t) {}
+
+typedef unsigned long long u64;
+
+constexpr int F_PY = 4;        // rows per lane
+constexpr int F_RING = 4;      // field-plane ring depth (prefetch distance 3)
+constexpr int F_SRING = 8;     // state-plane ring depth (a plane is used by NL consecutive iterations)
+constexpr int F_MAXNL = 4;
+
+struct FusedArgs {
+    const float *src[3];       // current field buffers [batch][nz][ny][nx]
+    float *dst[3];             // other ping-pong buffers
+    const uint8_t *state;
+    int nx, ny, nz, batch;
+    float lam[3];
+    float lut[3][32];          // source term by (state & 31): rate[s][mode] if kind in 1..4 else 0  [D G4]
+    int always_slow[3];        // 1: the clamp cannot be proven idle for this lambda -> always take the full path
+    float zero;                // 0.0f, opaque to ptxas (see Fused::level)
+};
+
+// ---- packed f32x2 arithmetic (Blackwell FADD2/FMUL2/FFMA2); .rn, no ftz: identical to two scalar ops ----
+__device__ __forceinline__ u64 pk(float lo, float hi) { u64 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ void upk(u64 v, float &lo, float &hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ u64 add2(u64 a, u64 b) { u64 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ u64 sub2(u64 a, u64 b) { u64 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ u64 mul2(u64 a, u64 b) { u64 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) { u64 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+
+// ---- mbarrier / bulk-copy helpers (shared::cta addresses as 32-bit) ----
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) { asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count)); }
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) { asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory"); }
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t}" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+
+__device__ __forceinline__ u64 lds64(uint32_t a) { u64 v; asm volatile("ld.shared.b64 %0, [%1];" : "=l"(v) : "r"(a)); return v; }
+__device__ __forceinline__ void sts64(uint32_t a, u64 v) { asm volatile("st.shared.b64 [%0], %1;" ::"r"(a), "l"(v) : "memory"); }
+__device__ __forceinline__ uint32_t lds16(uint32_t a) { uint32_t v; asm volatile("ld.shared.u16 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
+__device__ __forceinline__ float lds32f(uint32_t a) { float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a)); return v; }
+
+// per-thread view of one segment (unit = simulation x species, planes [za, zb))
+struct FusedCtx {
+    const float *src;          // field of this unit, already offset to this lane's (x0, y0)
+    float *dst;
+    const float *src_plane0;   // unit base (for the bulk copies)
+    const uint8_t *st_plane0;
+    int nx, nxny, nz;
+    int za, zb, t0, nsteps;
+    int ld_lo, ld_hi;          // planes level 0 loads
+    uint32_t itg;              // global iteration counter of this CTA (ring slots / mbarrier parities)
+    uint32_t flags, slowmask;  // bit k: "cells in my strip" for the plane level k works on
+    uint32_t bars, in_ring, st_ring, exch, lut;   // shared-memory addresses
+    uint32_t plane_bytes, st_bytes;
+    uint32_t lane_in_off, lane_st_off;            // this lane's offset inside a plane (bytes)
+    uint32_t ex_self, ex_up, ex_dn, ex_lvl, ex_buf;   // exchange addressing (bytes)
+    u64 lam2[F_PY];
+    u64 zero2;                 // (0, 0) that ptxas cannot see through
+    uint32_t rowmask;          // bit j: row y0+j exists and this lane's x pair is inside the lattice
+};
+
+template <int NL, int LRP>
+struct Fused {
+    // one sub-step of [D S1] for this lane's 2 x 4 points; C = centre plane, M/P = planes z-1/z+1 (same level)
+    template <bool SLOW>
+    static __device__ __forceinline__ void level(const u64 (&M)[F_PY], const u64 (&C)[F_PY], const u64 (&P)[F_PY], u64 (&N)[F_PY],
+                                                 u64 up, u64 dn, const u64 (&lam2)[F_PY], const u64 (&r2)[F_PY], const u64 zero2)
+    {
+        const u64 six2 = pk(6.0f, 6.0f);
+#pragma unroll
+        for (int j = 0; j < F_PY; ++j) {
+            float c0, c1;
+            upk(C[j], c0, c1);
+            const float xl = __shfl_up_sync(0xFFFFFFFFu, c1, 1, LRP);      // value at x0-1 (own c1 at the strip edge: WALL side, unused)
+            const float xr = __shfl_down_sync(0xFFFFFFFFu, c0, 1, LRP);    // value at x0+2
+            const u64 xs = pk(__fadd_rn(xl, c1), __fadd_rn(c0, xr));       // xm + xp
+            const u64 ys = add2(j == 0 ? up : C[j > 0 ? j - 1 : 0], j == F_PY - 1 ? dn : C[j < F_PY - 1 ? j + 1 : 0]);   // ym + yp
+            const u64 zs = add2(M[j], P[j]);                                 // zm + zp
+            const u64 s6 = add2(add2(xs, ys), zs);
+            // 6*c must be rounded on its own [D S1].  ptxas contracts mul.rn.f32x2 + sub.rn.f32x2 into one FFMA2 (seen in SASS,
+            // CUDA 12.9), so the product is formed as fma(6, c, 0) with a zero the compiler cannot fold: same value, same pipe cost.
+            const u64 lap = sub2(s6, fma2(six2, C[j], zero2));
+            u64 v = fma2(lam2[j], lap, C[j]);
+            if (SLOW) {
+                v = add2(v, r2[j]);
+                float a, b;
+                upk(v, a, b);
+                v = pk(fmaxf(a, 0.0f), fmaxf(b, 0.0f));
+            }
+            N[j] = v;
+        }
+    }
+
+    static __device__ __forceinline__ void issue(const FusedCtx &c, int i)
+    {
+        const uint32_t q = c.itg + (uint32_t)i;
+        const int t = c.t0 + i;
+        const uint32_t bar = c.bars + 8u * (q & (F_RING - 1));
+        if (t >= c.ld_lo && t < c.ld_hi) {
+            mbar_expect_tx(bar, c.plane_bytes + c.st_bytes);
+            bulk_g2s(c.in_ring + (q & (F_RING - 1)) * c.plane_bytes, c.src_plane0 + (size_t)t * c.nxny, c.plane_bytes, bar);
+            bulk_g2s(c.st_ring + (q & (F_SRING - 1)) * c.st_bytes, c.st_plane0 + (size_t)t * c.nxny, c.st_bytes, bar);
+        } else {
+            mbar_arrive(bar);
+        }
+    }
+
+    // level K (sub-step K) at iteration i: computes plane t-K, or copies a WALL plane, or idles
+    template <int PH, int K>
+    static __device__ __forceinline__ void levels(const int i, const int t, const uint32_t q, const uint32_t exr, const uint32_t exw,
+                                                  u64 (&h)[NL][3][F_PY], FusedCtx &c)
+    {
+        if constexpr (K <= NL) {
+            constexpr int sm = (PH - K - 1 + 12) % 3, sc = (PH - K + 12) % 3, sp = (PH - K + 1 + 12) % 3;
+            constexpr int KO = K < NL ? K : 0;                              // output level (unused when K == NL)
+            const int zc = t - K;
+            const int lo = max(1, c.za - (NL - K)), hi = min(c.nz - 1, c.zb + (NL - K));
+            if (zc >= lo && zc < hi) {
+                const u64 up = lds64(exr + (uint32_t)(K - 1) * c.ex_lvl + c.ex_up);
+                const u64 dn = lds64(exr + (uint32_t)(K - 1) * c.ex_lvl + c.ex_dn);
+                u64 r2[F_PY];
+                u64 nloc[F_PY];
+                u64 (&N)[F_PY] = *(K < NL ? &h[KO][sc] : &nloc);
+                if (((c.flags | c.slowmask) >> K) & 1u) {
+                    const uint32_t s = c.st_ring + ((q - (uint32_t)K) & (F_SRING - 1)) * c.st_bytes + c.lane_st_off;
+#pragma unroll
+                    for (int j = 0; j < F_PY; ++j) {
+                        const uint32_t w = ((c.rowmask >> j) & 1u) ? lds16(s + (uint32_t)(j * c.nx)) : 0u;
+                        r2[j] = pk(lds32f(c.lut + (w & 31u) * 4u), lds32f(c.lut + ((w >> 8) & 31u) * 4u));
+                    }
+                    level<true>(h[K - 1][sm], h[K - 1][sc], h[K - 1][sp], N, up, dn, c.lam2, r2, c.zero2);
+                } else {
+#pragma unroll
+                    for (int j = 0; j < F_PY; ++j) r2[j] = 0ull;
+                    level<false>(h[K - 1][sm], h[K - 1][sc], h[K - 1][sp], N, up, dn, c.lam2, r2, c.zero2);
+                }
+                if constexpr (K < NL) {
+                    sts64(exw + (uint32_t)K * c.ex_lvl + c.ex_self, N[0]);
+                    sts64(exw + (uint32_t)K * c.ex_lvl + c.ex_self + c.ex_lvl / 2, N[F_PY - 1]);
+                } else {
+                    float *o = c.dst + (size_t)zc * c.nxny;
+#pragma unroll
+                    for (int j = 0; j < F_PY; ++j)
+                        if ((c.rowmask >> j) & 1u) {
+                            float a, b;
+                            upk(N[j], a, b);
+                            *reinterpret_cast<float2 *>(o + j * c.nx) = make_float2(a, b);
+                        }
+                }
+            } else if (K < NL && (zc == 0 || zc == c.nz - 1) && zc >= c.za - (NL - K) && zc < c.zb + (NL - K)) {
+                // WALL plane: every level equals the input there
+                const float *p = c.src + (size_t)zc * c.nxny;
+#pragma unroll
+                for (int j = 0; j < F_PY; ++j) {
+                    float2 v = make_float2(0.0f, 0.0f);
+                    if ((c.rowmask >> j) & 1u) v = *reinterpret_cast<const float2 *>(p + j * c.nx);
+                    h[KO][sc][j] = pk(v.x, v.y);
+                }
+            }
+            levels<PH, K + 1>(i, t, q, exr, exw, h, c);
+        }
+    }
+
+    // one march iteration; PH = i mod 3 selects the register slots (slot of plane z = (z - t0) mod 3 on every level)
+    template <int PH>
+    static __device__ __forceinline__ void step(const int i, u64 (&h)[NL][3][F_PY], FusedCtx &c)
+    {
+        const int t = c.t0 + i;
+        const uint32_t q = c.itg + (uint32_t)i;
+        if (threadIdx.x == 0 && i + (F_RING - 1) < c.nsteps) issue(c, i + (F_RING - 1));
+        const uint32_t exr = c.exch + ((uint32_t)(i + 1) & 1u) * c.ex_buf;    // rows written by the previous iteration
+        const uint32_t exw = c.exch + ((uint32_t)i & 1u) * c.ex_buf;
+        // ---- level 0: plane t from the ring
+        mbar_wait(c.bars + 8u * (q & (F_RING - 1)), (q / F_RING) & 1u);
+        uint32_t cells = 0;
+        if (t >= c.ld_lo && t < c.ld_hi) {
+            const uint32_t a = c.in_ring + (q & (F_RING - 1)) * c.plane_bytes + c.lane_in_off;
+            const uint32_t s = c.st_ring + (q & (F_SRING - 1)) * c.st_bytes + c.lane_st_off;
+#pragma unroll
+            for (int j = 0; j < F_PY; ++j) {
+                const bool ok = (c.rowmask >> j) & 1u;
+                h[0][PH][j] = ok ? lds64(a + (uint32_t)(j * c.nx) * 4u) : 0ull;
+                const uint32_t w = ok ? lds16(s + (uint32_t)(j * c.nx)) : 0u;
+                cells |= ((w & 0x0707u) + 0x0101u) & 0x0606u;                // some byte has kind in 1..6
+            }
+            sts64(exw + c.ex_self, h[0][PH][0]);
+            sts64(exw + c.ex_self + c.ex_lvl / 2, h[0][PH][F_PY - 1]);
+        }
+        c.flags = (c.flags << 1) | (__any_sync(0xFFFFFFFFu, cells != 0u) ? 1u : 0u);
+        // ---- levels 1..NL: level k computes plane t-k from level k-1
+        levels<PH, 1>(i, t, q, exr, exw, h, c);
+        __syncthreads();
+    }
+};
+
+struct FusedGeom {             // host-computed launch geometry, passed by value
+    int nwarps, ngroups_alloc; // strips of F_PY rows: groups = nwarps * (32 / LRP)
+    uint32_t off_lut, off_in, off_st, off_ex, smem_bytes;
+    long long total_planes;    // batch * 3 * (nz - 2): the flattened (unit, interior plane) space
+};
+
+template <int NL, int LRP>
+__global__ void __launch_bounds__(512, 1) k_diffuse_fused(const FusedArgs A, const FusedGeom Gm)
+{
+    extern __shared__ __align__(128) unsigned char fsm[];
+    constexpr int RW = 32 / LRP;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int lx = lane % LRP, g = warp * RW + lane / LRP;
+    const int x0 = 2 * lx, y0 = F_PY * g;
+    const uint32_t base = smem_u32(fsm);
+
+    FusedCtx c;
+    c.nx = A.nx; c.nxny = A.nx * A.ny; c.nz = A.nz;
+    c.bars = base; c.lut = base + Gm.off_lut; c.in_ring = base + Gm.off_in; c.st_ring = base + Gm.off_st; c.exch = base + Gm.off_ex;
+    c.plane_bytes = (uint32_t)c.nxny * 4u; c.st_bytes = (uint32_t)c.nxny;
+    c.lane_in_off = (uint32_t)(y0 * A.nx + x0) * 4u; c.lane_st_off = (uint32_t)(y0 * A.nx + x0);
+    const uint32_t grp_bytes = LRP * 8u;
+    c.ex_lvl = 2u * (uint32_t)(Gm.ngroups_alloc + 2) * grp_bytes;            // [top rows | bottom rows], each with a zero group at both ends
+    c.ex_buf = NL * c.ex_lvl;
+    c.ex_self = (uint32_t)(g + 1) * grp_bytes + (uint32_t)lx * 8u;           // my slot in the "top rows" array
+    c.ex_up = c.ex_lvl / 2 + (uint32_t)g * grp_bytes + (uint32_t)lx * 8u;     // bottom row of the strip above
+    c.ex_dn = (uint32_t)(g + 2) * grp_bytes + (uint32_t)lx * 8u;              // top row of the strip below
+    c.rowmask = 0;
+#pragma unroll
+    for (int j = 0; j < F_PY; ++j)
+        if (y0 + j < A.ny && x0 < A.nx) c.rowmask |= 1u << j;
+    c.itg = 0;
+    c.zero2 = pk(A.zero, A.zero);
+
+    // one-time shared-memory setup: barriers, source-term tables, zeroed exchange (its end groups stay zero)
+    if (tid == 0) {
+#pragma unroll
+        for (int r = 0; r < F_RING; ++r) mbar_init(c.bars + 8u * r, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    for (int e = tid; e < 96; e += blockDim.x) reinterpret_cast<float *>(fsm + Gm.off_lut)[e] = A.lut[e / 32][e % 32];
+    for (uint32_t e = tid; e < 2u * c.ex_buf / 8u; e += blockDim.x) reinterpret_cast<u64 *>(fsm + Gm.off_ex)[e] = 0ull;
+    __syncthreads();
+
+    const int nzi = A.nz - 2;
+    long long p = Gm.total_planes * (long long)blockIdx.x / gridDim.x;
+    const long long p_end = Gm.total_planes * (long long)(blockIdx.x + 1) / gridDim.x;
+    u64 h[NL][3][F_PY];
+#pragma unroll
+    for (int k = 0; k < NL; ++k)
+#pragma unroll
+        for (int s = 0; s < 3; ++s)
+#pragma unroll
+            for (int j = 0; j < F_PY; ++j) h[k][s][j] = 0ull;
+
+    while (p < p_end) {
+        const int unit = (int)(p / nzi);
+        const int b = unit / 3, sp = unit % 3;
+        c.za = 1 + (int)(p - (long long)unit * nzi);
+        c.zb = (int)min((long long)(A.nz - 1), (long long)c.za + (p_end - p));
+        p += c.zb - c.za;
+        const size_t ubase = (size_t)b * (size_t)c.nxny * (size_t)A.nz;
+        c.src_plane0 = A.src[sp] + ubase;
+        c.st_plane0 = A.state + ubase;
+        c.src = c.src_plane0 + (y0 * A.nx + x0);
+        c.dst = A.dst[sp] + ubase + (y0 * A.nx + x0);
+        c.t0 = c.za - NL;
+        c.nsteps = c.zb - c.za + 2 * NL;
+        c.ld_lo = max(0, c.za - NL); c.ld_hi = min(A.nz, c.zb + NL);
+        c.flags = 0; c.slowmask = A.always_slow[sp] ? 0xFFFFFFFFu : 0u;
+        c.lut = base + Gm.off_lut + (uint32_t)sp * 128u;
+        const float lam = A.lam[sp];
+#pragma unroll
+        for (int j = 0; j < F_PY; ++j) {
+            const int y = y0 + j;
+            const bool rowin = y > 0 && y < A.ny - 1;                          // y walls and rows outside the lattice: lambda = 0
+            c.lam2[j] = pk(rowin && x0 > 0 && x0 < A.nx - 1 ? lam : 0.0f, rowin && x0 + 1 < A.nx - 1 ? lam : 0.0f);
+        }
+        if (tid == 0)
+            for (int i = 0; i < F_RING - 1 && i < c.nsteps; ++i) Fused<NL, LRP>::issue(c, i);
+        for (int i = 0; i < c.nsteps; i += 3) {
+            Fused<NL, LRP>::template step<0>(i, h, c);
+            if (i + 1 < c.nsteps) Fused<NL, LRP>::template step<1>(i + 1, h, c);
+            if (i + 2 < c.nsteps) Fused<NL, LRP>::template step<2>(i + 2, h, c);
+        }
+        c.itg += (uint32_t)c.nsteps;
+    }
+}
+
+// ------------------------------------------------------------------ host side --
+struct FusedPlan {
+    bool ok = false;
+    int lrp = 0, sms = 0;
+    FusedGeom geom{};
+    FusedArgs args{};
+    int npass = 0, pass_nl[2] = { 0, 0 };
+};
+
+inline size_t fused_smem(int nx, int ny, int nl, int lrp, FusedGeom &G)
+{
+    const int rw = 32 / lrp, groups = (ny + F_PY - 1) / F_PY;
+    G.nwarps = (groups + rw - 1) / rw;
+    G.ngroups_alloc = G.nwarps * rw;
+    size_t o = 128;
+    G.off_lut = (uint32_t)o; o += 96 * 4; o = (o + 127) / 128 * 128;
+    G.off_in = (uint32_t)o; o += (size_t)F_RING * nx * ny * 4; o = (o + 127) / 128 * 128;
+    G.off_st = (uint32_t)o; o += (size_t)F_SRING * nx * ny; o = (o + 127) / 128 * 128;
+    G.off_ex = (uint32_t)o; o += (size_t)2 * nl * 2 * (G.ngroups_alloc + 2) * lrp * 8;
+    G.smem_bytes = (uint32_t)o;
+    return o;
+}
+
+template <int NL, int LRP>
+inline cudaError_t fused_launch_t(const FusedArgs &A, FusedGeom G, int grid, cudaStream_t st)
+{
+    fused_smem(A.nx, A.ny, NL, LRP, G);
+    G.total_planes = (long long)A.batch * 3 * (A.nz - 2);
+    static bool attr_done = false;      // per instantiation
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(k_diffuse_fused<NL, LRP>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    k_diffuse_fused<NL, LRP><<<grid, G.nwarps * 32, G.smem_bytes, st>>>(A, G);
+    return cudaGetLastError();
+}
+
+// Decide whether the fused kernel covers this lattice, and precompute its arguments.
+inline void fused_configure(const KParams &P, FusedPlan &F)
+{
+    F.ok = false;
+    if (P.nx % 2 || P.nx > 64 || P.nx < 4 || P.nz < 3 || (P.nx * P.ny) % 16 || P.n_sub < 1 || P.n_sub > 2 * F_MAXNL) return;
+    F.lrp = P.nx <= 32 ? 16 : 32;
+    FusedGeom G{};
+    if (fused_smem(P.nx, P.ny, F_MAXNL, F.lrp, G) > 227 * 1024 || G.nwarps > 16) return;
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return;
+    F.sms = prop.multiProcessorCount;
+    F.args.zero = 0.0f;
+    F.args.nx = P.nx; F.args.ny = P.ny; F.args.nz = P.nz; F.args.batch = P.batch;
+    for (int s = 0; s < 3; ++s) {
+        F.args.lam[s] = P.lambda[s];
+        // without a source term v = c + lambda*(sum6 - RN(6c)) >= c*(1 - 6*lambda*(1 + 2^-24)) >= 0 needs this margin
+        F.args.always_slow[s] = !((double)P.lambda[s] * 6.0 * (1.0 + 1.0 / 8388608.0) <= 1.0);
+        for (int e = 0; e < 32; ++e) {
+            const int kind = e & 7, mode = e >> 3;
+            F.args.lut[s][e] = (kind >= 1 && kind <= 4) ? P.rate[s][mode] : 0.0f;
+        }
+    }
+    if (P.n_sub <= F_MAXNL) { F.npass = 1; F.pass_nl[0] = P.n_sub; }
+    else { F.npass = 2; F.pass_nl[0] = (P.n_sub + 1) / 2; F.pass_nl[1] = P.n_sub / 2; }
+    F.ok = true;
+}
+
+inline bool fused_supported(const FusedPlan &F) { return F.ok; }
+
+// Enqueue all n_sub sub-steps starting from ping-pong buffer `cur`; returns the number of passes (= buffer flips).
+inline int launch_fused(FusedPlan &F, const Lattice &L, int cur, cudaStream_t st, cudaError_t *err)
+{
+    *err = cudaSuccess;
+    for (int ps = 0; ps < F.npass; ++ps) {
+        FusedArgs A = F.args;
+        for (int s = 0; s < 3; ++s) { A.src[s] = L.f[cur][s]; A.dst[s] = L.f[cur ^ 1][s]; }
+        A.state = L.state;
+        FusedGeom G{};
+        // CTAs per SM: the 512-thread (nx > 32) kernel fills an SM; smaller lattices use several CTAs per SM
+        fused_smem(A.nx, A.ny, F.pass_nl[ps], F.lrp, G);
+        const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(std::min<size_t>(4, (227 * 1024) / (G.smem_bytes + 1024)), 512 / (G.nwarps * 32)));
+        const long long total = (long long)A.batch * 3 * (A.nz - 2);
+        const int grid = (int)std::max<long long>(1, std::min<long long>((long long)F.sms * per_sm, total / 2 + 1));
+        cudaError_t e;
+        const int nl = F.pass_nl[ps];
+#define CA_FUSED_CASE(NLV) case NLV: e = (F.lrp == 16) ? fused_launch_t<NLV, 16>(A, G, grid, st) : fused_launch_t<NLV, 32>(A, G, grid, st); break;
+        switch (nl) {
+            CA_FUSED_CASE(1) CA_FUSED_CASE(2) CA_FUSED_CASE(3) CA_FUSED_CASE(4)
+        default: e = cudaErrorInvalidValue;
+        }
+#undef CA_FUSED_CASE
+        if (e != cudaSuccess) { *err = e; return ps; }
+        cur ^= 1;
+    }
+    return F.npass;
+}
+
 }  // namespace ca
