@@ -12,7 +12,7 @@
 //     along z; a lane owns 2 (x) x 4 (y) points of the plane, a warp a 64 x 4 strip (two 32 x 4 strips
 //     when nx <= 32);
 //   * input planes and state planes arrive by bulk async copy (TMA 1-D, UBLKCP) into shared-memory rings,
-//     completion on mbarriers, 3 planes ahead;
+//     completion on mbarriers, 2 planes ahead;
 //   * level k (sub-step k) computes plane t-k while level 0 loads plane t: each level keeps 3 planes of its
 //     input level in registers (ring of 3, the march loop is unrolled by 3 so that no register is moved);
 //   * x-neighbours come from the neighbouring lane by shuffle, y-neighbours across strips through a small
@@ -32,7 +32,7 @@ namespace ca {
 typedef unsigned long long u64;
 
 constexpr int F_PY = 4;        // rows per lane
-constexpr int F_RING = 4;      // field-plane ring depth (prefetch distance 3)
+constexpr int F_RING = 3;      // field-plane ring depth = register phase count (prefetch distance 2)
 constexpr int F_SRING = 8;     // state-plane ring depth (a plane is used by NL consecutive iterations)
 constexpr int F_MAXNL = 4;
 
@@ -84,28 +84,50 @@ __device__ __forceinline__ void sts64(uint32_t a, u64 v) { asm volatile("st.shar
 __device__ __forceinline__ uint32_t lds16(uint32_t a) { uint32_t v; asm volatile("ld.shared.u16 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
 __device__ __forceinline__ float lds32f(uint32_t a) { float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a)); return v; }
 
+struct FusedGeom {             // host-computed launch geometry, passed by value
+    int nwarps, ngroups_alloc; // strips of F_PY rows: groups = nwarps * (32 / LRP)
+    uint32_t off_lut, off_in, off_st, off_ex, smem_bytes;
+    long long total_planes;    // batch * 3 * (nz - 2): the flattened (unit, interior plane) space
+};
+
 // per-thread view of one segment (unit = simulation x species, planes [za, zb))
 struct FusedCtx {
     const float *src;          // field of this unit, already offset to this lane's (x0, y0)
     float *dst;
     const float *src_plane0;   // unit base (for the bulk copies)
     const uint8_t *st_plane0;
-    int nx, nxny, nz;
+    int nx, nxny, nz;          // run-time geometry (ignored by the fixed-size instantiations)
+    uint32_t ex_lvl;
     int za, zb, t0, nsteps;
     int ld_lo, ld_hi;          // planes level 0 loads
-    uint32_t itg;              // global iteration counter of this CTA (ring slots / mbarrier parities)
+    int st_lo, st_hi;          // iterations [st_lo, st_hi): every level computes, no WALL plane involved
+    uint32_t itg;              // running iteration counter of this CTA (state-ring slots)
+    uint32_t par;              // bit r: parity to wait for on field-ring slot r
     uint32_t flags, slowmask;  // bit k: "cells in my strip" for the plane level k works on
-    uint32_t bars, in_ring, st_ring, exch, lut;   // shared-memory addresses
-    uint32_t plane_bytes, st_bytes;
-    uint32_t lane_in_off, lane_st_off;            // this lane's offset inside a plane (bytes)
-    uint32_t ex_self, ex_up, ex_dn, ex_lvl, ex_buf;   // exchange addressing (bytes)
+    uint32_t bars, in_ring, st_ring, lut;         // shared-memory addresses
+    uint32_t in_lane;          // this lane's (x0, y0) inside ring slot 0
+    uint32_t st_lane, st_strip;   // this lane's points / this lane's 8 bytes of the warp strip inside state slot 0
+    uint32_t ex_self;          // this lane's slot in the "top rows" array of exchange buffer 0, level 0
     u64 lam2[F_PY];
     u64 zero2;                 // (0, 0) that ptxas cannot see through
     uint32_t rowmask;          // bit j: row y0+j exists and this lane's x pair is inside the lattice
+    bool strip_ok;
 };
 
-template <int NL, int LRP>
+// NX = NY = 0: lattice dims at run time (any even nx <= 2*LRP); otherwise compile-time dims, all address math folds
+template <int NL, int LRP, int NX, int NY>
 struct Fused {
+    static constexpr bool FIXED = NX != 0;
+    static constexpr int RW = 32 / LRP;
+    static constexpr bool FULL = FIXED && NX == 2 * LRP && NY % (F_PY * RW) == 0;    // every lane and row is inside the lattice
+    static constexpr uint32_t GRP = LRP * 8u;                                         // bytes of one exchanged row
+    static constexpr uint32_t EXL = FIXED ? 2u * (((NY + F_PY * RW - 1) / (F_PY * RW)) * RW + 2u) * GRP : 0u;
+
+    static __device__ __forceinline__ int nx(const FusedCtx &c) { return FIXED ? NX : c.nx; }
+    static __device__ __forceinline__ int nxny(const FusedCtx &c) { return FIXED ? NX * NY : c.nxny; }
+    static __device__ __forceinline__ uint32_t exl(const FusedCtx &c) { return FIXED ? EXL : c.ex_lvl; }
+    static __device__ __forceinline__ bool row(const FusedCtx &c, int j) { return FULL ? true : ((c.rowmask >> j) & 1u) != 0u; }
+
     // one sub-step of [D S1] for this lane's 2 x 4 points; C = centre plane, M/P = planes z-1/z+1 (same level)
     template <bool SLOW>
     static __device__ __forceinline__ void level(const u64 (&M)[F_PY], const u64 (&C)[F_PY], const u64 (&P)[F_PY], u64 (&N)[F_PY],
@@ -136,41 +158,44 @@ struct Fused {
         }
     }
 
-    static __device__ __forceinline__ void issue(const FusedCtx &c, int i)
+    // producer (one thread): start the bulk copies of iteration i into field-ring slot i mod 3
+    static __device__ __forceinline__ void issue(const FusedCtx &c, int i, int slot)
     {
-        const uint32_t q = c.itg + (uint32_t)i;
         const int t = c.t0 + i;
-        const uint32_t bar = c.bars + 8u * (q & (F_RING - 1));
+        const uint32_t bar = c.bars + 8u * (uint32_t)slot;
+        const uint32_t pb = (uint32_t)nxny(c) * 4u, sb = (uint32_t)nxny(c);
         if (t >= c.ld_lo && t < c.ld_hi) {
-            mbar_expect_tx(bar, c.plane_bytes + c.st_bytes);
-            bulk_g2s(c.in_ring + (q & (F_RING - 1)) * c.plane_bytes, c.src_plane0 + (size_t)t * c.nxny, c.plane_bytes, bar);
-            bulk_g2s(c.st_ring + (q & (F_SRING - 1)) * c.st_bytes, c.st_plane0 + (size_t)t * c.nxny, c.st_bytes, bar);
+            mbar_expect_tx(bar, pb + sb);
+            bulk_g2s(c.in_ring + (uint32_t)slot * pb, c.src_plane0 + (size_t)t * nxny(c), pb, bar);
+            bulk_g2s(c.st_ring + ((c.itg + (uint32_t)i) & (F_SRING - 1)) * sb, c.st_plane0 + (size_t)t * nxny(c), sb, bar);
         } else {
             mbar_arrive(bar);
         }
     }
 
-    // level K (sub-step K) at iteration i: computes plane t-K, or copies a WALL plane, or idles
-    template <int PH, int K>
-    static __device__ __forceinline__ void levels(const int i, const int t, const uint32_t q, const uint32_t exr, const uint32_t exw,
+    // level K (sub-step K) at iteration i: computes plane t-K; outside the steady range it may idle or copy a WALL plane
+    template <int PH, int K, bool STEADY>
+    static __device__ __forceinline__ void levels(const int t, const uint32_t q, const uint32_t exr, const uint32_t exw,
                                                   u64 (&h)[NL][3][F_PY], FusedCtx &c)
     {
         if constexpr (K <= NL) {
             constexpr int sm = (PH - K - 1 + 12) % 3, sc = (PH - K + 12) % 3, sp = (PH - K + 1 + 12) % 3;
             constexpr int KO = K < NL ? K : 0;                              // output level (unused when K == NL)
             const int zc = t - K;
-            const int lo = max(1, c.za - (NL - K)), hi = min(c.nz - 1, c.zb + (NL - K));
-            if (zc >= lo && zc < hi) {
-                const u64 up = lds64(exr + (uint32_t)(K - 1) * c.ex_lvl + c.ex_up);
-                const u64 dn = lds64(exr + (uint32_t)(K - 1) * c.ex_lvl + c.ex_dn);
+            bool compute = true;
+            if (!STEADY) compute = zc >= max(1, c.za - (NL - K)) && zc < min(c.nz - 1, c.zb + (NL - K));
+            if (compute) {
+                const uint32_t el = exl(c);
+                const u64 up = lds64(exr + (uint32_t)(K - 1) * el + (el / 2 - GRP));     // bottom row of the strip above
+                const u64 dn = lds64(exr + (uint32_t)(K - 1) * el + GRP);                // top row of the strip below
                 u64 r2[F_PY];
                 u64 nloc[F_PY];
                 u64 (&N)[F_PY] = *(K < NL ? &h[KO][sc] : &nloc);
                 if (((c.flags | c.slowmask) >> K) & 1u) {
-                    const uint32_t s = c.st_ring + ((q - (uint32_t)K) & (F_SRING - 1)) * c.st_bytes + c.lane_st_off;
+                    const uint32_t s = c.st_lane + ((q - (uint32_t)K) & (F_SRING - 1)) * (uint32_t)nxny(c);
 #pragma unroll
                     for (int j = 0; j < F_PY; ++j) {
-                        const uint32_t w = ((c.rowmask >> j) & 1u) ? lds16(s + (uint32_t)(j * c.nx)) : 0u;
+                        const uint32_t w = row(c, j) ? lds16(s + (uint32_t)(j * nx(c))) : 0u;
                         r2[j] = pk(lds32f(c.lut + (w & 31u) * 4u), lds32f(c.lut + ((w >> 8) & 31u) * 4u));
                     }
                     level<true>(h[K - 1][sm], h[K - 1][sc], h[K - 1][sp], N, up, dn, c.lam2, r2, c.zero2);
@@ -180,96 +205,91 @@ struct Fused {
                     level<false>(h[K - 1][sm], h[K - 1][sc], h[K - 1][sp], N, up, dn, c.lam2, r2, c.zero2);
                 }
                 if constexpr (K < NL) {
-                    sts64(exw + (uint32_t)K * c.ex_lvl + c.ex_self, N[0]);
-                    sts64(exw + (uint32_t)K * c.ex_lvl + c.ex_self + c.ex_lvl / 2, N[F_PY - 1]);
+                    sts64(exw + (uint32_t)K * el, N[0]);
+                    sts64(exw + (uint32_t)K * el + el / 2, N[F_PY - 1]);
                 } else {
-                    float *o = c.dst + (size_t)zc * c.nxny;
+                    float *o = c.dst + (size_t)zc * nxny(c);
 #pragma unroll
                     for (int j = 0; j < F_PY; ++j)
-                        if ((c.rowmask >> j) & 1u) {
+                        if (row(c, j)) {
                             float a, b;
                             upk(N[j], a, b);
-                            *reinterpret_cast<float2 *>(o + j * c.nx) = make_float2(a, b);
+                            *reinterpret_cast<float2 *>(o + j * nx(c)) = make_float2(a, b);
                         }
                 }
             } else if (K < NL && (zc == 0 || zc == c.nz - 1) && zc >= c.za - (NL - K) && zc < c.zb + (NL - K)) {
                 // WALL plane: every level equals the input there
-                const float *p = c.src + (size_t)zc * c.nxny;
+                const float *p = c.src + (size_t)zc * nxny(c);
 #pragma unroll
                 for (int j = 0; j < F_PY; ++j) {
                     float2 v = make_float2(0.0f, 0.0f);
-                    if ((c.rowmask >> j) & 1u) v = *reinterpret_cast<const float2 *>(p + j * c.nx);
+                    if (row(c, j)) v = *reinterpret_cast<const float2 *>(p + j * nx(c));
                     h[KO][sc][j] = pk(v.x, v.y);
                 }
             }
-            levels<PH, K + 1>(i, t, q, exr, exw, h, c);
+            levels<PH, K + 1, STEADY>(t, q, exr, exw, h, c);
         }
     }
 
-    // one march iteration; PH = i mod 3 selects the register slots (slot of plane z = (z - t0) mod 3 on every level)
-    template <int PH>
+    // one march iteration; PH = i mod 3 selects the field-ring slot and the register slots
+    // (slot of plane z = (z - t0) mod 3 on every level)
+    template <int PH, bool STEADY>
     static __device__ __forceinline__ void step(const int i, u64 (&h)[NL][3][F_PY], FusedCtx &c)
     {
         const int t = c.t0 + i;
         const uint32_t q = c.itg + (uint32_t)i;
-        if (threadIdx.x == 0 && i + (F_RING - 1) < c.nsteps) issue(c, i + (F_RING - 1));
-        const uint32_t exr = c.exch + ((uint32_t)(i + 1) & 1u) * c.ex_buf;    // rows written by the previous iteration
-        const uint32_t exw = c.exch + ((uint32_t)i & 1u) * c.ex_buf;
+        if (threadIdx.x == 0 && i + (F_RING - 1) < c.nsteps) issue(c, i + (F_RING - 1), (PH + F_RING - 1) % 3);
+        const uint32_t exb = exl(c) * NL;                                   // bytes of one exchange buffer
+        const uint32_t exw = c.ex_self + ((uint32_t)i & 1u) * exb;          // rows written now, read by the next iteration
+        const uint32_t exr = c.ex_self + exb - ((uint32_t)i & 1u) * exb;    // rows written by the previous iteration
         // ---- level 0: plane t from the ring
-        mbar_wait(c.bars + 8u * (q & (F_RING - 1)), (q / F_RING) & 1u);
-        uint32_t cells = 0;
-        if (t >= c.ld_lo && t < c.ld_hi) {
-            const uint32_t a = c.in_ring + (q & (F_RING - 1)) * c.plane_bytes + c.lane_in_off;
-            const uint32_t s = c.st_ring + (q & (F_SRING - 1)) * c.st_bytes + c.lane_st_off;
+        mbar_wait(c.bars + 8u * PH, (c.par >> PH) & 1u);
+        c.par ^= 1u << PH;
+        bool any = false;
+        if (STEADY || (t >= c.ld_lo && t < c.ld_hi)) {
+            const uint32_t a = c.in_lane + (uint32_t)PH * (uint32_t)nxny(c) * 4u;
 #pragma unroll
-            for (int j = 0; j < F_PY; ++j) {
-                const bool ok = (c.rowmask >> j) & 1u;
-                h[0][PH][j] = ok ? lds64(a + (uint32_t)(j * c.nx) * 4u) : 0ull;
-                const uint32_t w = ok ? lds16(s + (uint32_t)(j * c.nx)) : 0u;
-                cells |= ((w & 0x0707u) + 0x0101u) & 0x0606u;                // some byte has kind in 1..6
-            }
-            sts64(exw + c.ex_self, h[0][PH][0]);
-            sts64(exw + c.ex_self + c.ex_lvl / 2, h[0][PH][F_PY - 1]);
+            for (int j = 0; j < F_PY; ++j) h[0][PH][j] = row(c, j) ? lds64(a + (uint32_t)(j * nx(c)) * 4u) : 0ull;
+            sts64(exw, h[0][PH][0]);
+            sts64(exw + exl(c) / 2, h[0][PH][F_PY - 1]);
+            // "cells in my strip": every lane looks at 8 bytes of the warp's strip of the state plane; a byte counts when kind is 1..6
+            const u64 w = c.strip_ok ? lds64(c.st_strip + (q & (F_SRING - 1)) * (uint32_t)nxny(c)) : 0ull;
+            any = (((w & 0x0707070707070707ull) + 0x0101010101010101ull) & 0x0606060606060606ull) != 0ull;
         }
-        c.flags = (c.flags << 1) | (__any_sync(0xFFFFFFFFu, cells != 0u) ? 1u : 0u);
+        c.flags = (c.flags << 1) | (__any_sync(0xFFFFFFFFu, any) ? 1u : 0u);
         // ---- levels 1..NL: level k computes plane t-k from level k-1
-        levels<PH, 1>(i, t, q, exr, exw, h, c);
+        levels<PH, 1, STEADY>(t, q, exr, exw, h, c);
         __syncthreads();
     }
 };
 
-struct FusedGeom {             // host-computed launch geometry, passed by value
-    int nwarps, ngroups_alloc; // strips of F_PY rows: groups = nwarps * (32 / LRP)
-    uint32_t off_lut, off_in, off_st, off_ex, smem_bytes;
-    long long total_planes;    // batch * 3 * (nz - 2): the flattened (unit, interior plane) space
-};
-
-template <int NL, int LRP>
+template <int NL, int LRP, int NX, int NY>
 __global__ void __launch_bounds__(512, 1) k_diffuse_fused(const FusedArgs A, const FusedGeom Gm)
 {
+    typedef Fused<NL, LRP, NX, NY> F;
     extern __shared__ __align__(128) unsigned char fsm[];
     constexpr int RW = 32 / LRP;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int lx = lane % LRP, g = warp * RW + lane / LRP;
     const int x0 = 2 * lx, y0 = F_PY * g;
     const uint32_t base = smem_u32(fsm);
+    const int nxr = NX ? NX : A.nx, nyr = NY ? NY : A.ny;
 
     FusedCtx c;
-    c.nx = A.nx; c.nxny = A.nx * A.ny; c.nz = A.nz;
-    c.bars = base; c.lut = base + Gm.off_lut; c.in_ring = base + Gm.off_in; c.st_ring = base + Gm.off_st; c.exch = base + Gm.off_ex;
-    c.plane_bytes = (uint32_t)c.nxny * 4u; c.st_bytes = (uint32_t)c.nxny;
-    c.lane_in_off = (uint32_t)(y0 * A.nx + x0) * 4u; c.lane_st_off = (uint32_t)(y0 * A.nx + x0);
-    const uint32_t grp_bytes = LRP * 8u;
-    c.ex_lvl = 2u * (uint32_t)(Gm.ngroups_alloc + 2) * grp_bytes;            // [top rows | bottom rows], each with a zero group at both ends
-    c.ex_buf = NL * c.ex_lvl;
-    c.ex_self = (uint32_t)(g + 1) * grp_bytes + (uint32_t)lx * 8u;           // my slot in the "top rows" array
-    c.ex_up = c.ex_lvl / 2 + (uint32_t)g * grp_bytes + (uint32_t)lx * 8u;     // bottom row of the strip above
-    c.ex_dn = (uint32_t)(g + 2) * grp_bytes + (uint32_t)lx * 8u;              // top row of the strip below
+    c.nx = nxr; c.nxny = nxr * nyr; c.nz = A.nz;
+    c.bars = base; c.in_ring = base + Gm.off_in; c.st_ring = base + Gm.off_st;
+    c.in_lane = c.in_ring + (uint32_t)(y0 * nxr + x0) * 4u;
+    c.st_lane = c.st_ring + (uint32_t)(y0 * nxr + x0);
+    const int strip_bytes = F_PY * RW * nxr;                                   // the warp's rows are contiguous in the plane
+    c.strip_ok = 8 * lane < strip_bytes && (warp * F_PY * RW) * nxr + 8 * lane + 8 <= nxr * nyr;
+    c.st_strip = c.st_ring + (uint32_t)((warp * F_PY * RW) * nxr + 8 * lane);
+    c.ex_lvl = 2u * (uint32_t)(Gm.ngroups_alloc + 2) * F::GRP;                  // [top rows | bottom rows], each with a zero group at both ends
+    c.ex_self = base + Gm.off_ex + (uint32_t)(g + 1) * F::GRP + (uint32_t)lx * 8u;
     c.rowmask = 0;
 #pragma unroll
     for (int j = 0; j < F_PY; ++j)
-        if (y0 + j < A.ny && x0 < A.nx) c.rowmask |= 1u << j;
-    c.itg = 0;
+        if (y0 + j < nyr && x0 < nxr) c.rowmask |= 1u << j;
+    c.itg = 0; c.par = 0;
     c.zero2 = pk(A.zero, A.zero);
 
     // one-time shared-memory setup: barriers, source-term tables, zeroed exchange (its end groups stay zero)
@@ -279,7 +299,7 @@ __global__ void __launch_bounds__(512, 1) k_diffuse_fused(const FusedArgs A, con
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     for (int e = tid; e < 96; e += blockDim.x) reinterpret_cast<float *>(fsm + Gm.off_lut)[e] = A.lut[e / 32][e % 32];
-    for (uint32_t e = tid; e < 2u * c.ex_buf / 8u; e += blockDim.x) reinterpret_cast<u64 *>(fsm + Gm.off_ex)[e] = 0ull;
+    for (uint32_t e = tid; e < 2u * NL * c.ex_lvl / 8u; e += blockDim.x) reinterpret_cast<u64 *>(fsm + Gm.off_ex)[e] = 0ull;
     __syncthreads();
 
     const int nzi = A.nz - 2;
@@ -302,26 +322,33 @@ __global__ void __launch_bounds__(512, 1) k_diffuse_fused(const FusedArgs A, con
         const size_t ubase = (size_t)b * (size_t)c.nxny * (size_t)A.nz;
         c.src_plane0 = A.src[sp] + ubase;
         c.st_plane0 = A.state + ubase;
-        c.src = c.src_plane0 + (y0 * A.nx + x0);
-        c.dst = A.dst[sp] + ubase + (y0 * A.nx + x0);
+        c.src = c.src_plane0 + (y0 * nxr + x0);
+        c.dst = A.dst[sp] + ubase + (y0 * nxr + x0);
         c.t0 = c.za - NL;
         c.nsteps = c.zb - c.za + 2 * NL;
         c.ld_lo = max(0, c.za - NL); c.ld_hi = min(A.nz, c.zb + NL);
+        c.st_lo = 2 * NL; c.st_hi = min(A.nz, c.zb + NL) - c.t0;              // za+NL <= t < min(nz, zb+NL)
         c.flags = 0; c.slowmask = A.always_slow[sp] ? 0xFFFFFFFFu : 0u;
         c.lut = base + Gm.off_lut + (uint32_t)sp * 128u;
         const float lam = A.lam[sp];
 #pragma unroll
         for (int j = 0; j < F_PY; ++j) {
             const int y = y0 + j;
-            const bool rowin = y > 0 && y < A.ny - 1;                          // y walls and rows outside the lattice: lambda = 0
-            c.lam2[j] = pk(rowin && x0 > 0 && x0 < A.nx - 1 ? lam : 0.0f, rowin && x0 + 1 < A.nx - 1 ? lam : 0.0f);
+            const bool rowin = y > 0 && y < nyr - 1;                           // y walls and rows outside the lattice: lambda = 0
+            c.lam2[j] = pk(rowin && x0 > 0 && x0 < nxr - 1 ? lam : 0.0f, rowin && x0 + 1 < nxr - 1 ? lam : 0.0f);
         }
         if (tid == 0)
-            for (int i = 0; i < F_RING - 1 && i < c.nsteps; ++i) Fused<NL, LRP>::issue(c, i);
+            for (int i = 0; i < F_RING - 1 && i < c.nsteps; ++i) F::issue(c, i, i);
         for (int i = 0; i < c.nsteps; i += 3) {
-            Fused<NL, LRP>::template step<0>(i, h, c);
-            if (i + 1 < c.nsteps) Fused<NL, LRP>::template step<1>(i + 1, h, c);
-            if (i + 2 < c.nsteps) Fused<NL, LRP>::template step<2>(i + 2, h, c);
+            if (i >= c.st_lo && i + 3 <= c.st_hi) {
+                F::template step<0, true>(i, h, c);
+                F::template step<1, true>(i + 1, h, c);
+                F::template step<2, true>(i + 2, h, c);
+            } else {
+                F::template step<0, false>(i, h, c);
+                if (i + 1 < c.nsteps) F::template step<1, false>(i + 1, h, c);
+                if (i + 2 < c.nsteps) F::template step<2, false>(i + 2, h, c);
+            }
         }
         c.itg += (uint32_t)c.nsteps;
     }
@@ -330,8 +357,7 @@ __global__ void __launch_bounds__(512, 1) k_diffuse_fused(const FusedArgs A, con
 // ------------------------------------------------------------------ host side --
 struct FusedPlan {
     bool ok = false;
-    int lrp = 0, sms = 0;
-    FusedGeom geom{};
+    int lrp = 0, sms = 0, fixed = 0;   // fixed: 0 run-time dims, 32 / 64: the cubic fast instantiations
     FusedArgs args{};
     int npass = 0, pass_nl[2] = { 0, 0 };
 };
@@ -350,19 +376,29 @@ inline size_t fused_smem(int nx, int ny, int nl, int lrp, FusedGeom &G)
     return o;
 }
 
-template <int NL, int LRP>
-inline cudaError_t fused_launch_t(const FusedArgs &A, FusedGeom G, int grid, cudaStream_t st)
+template <int NL, int LRP, int NX, int NY>
+inline cudaError_t fused_launch_t(const FusedArgs &A, int grid, cudaStream_t st)
 {
+    FusedGeom G{};
     fused_smem(A.nx, A.ny, NL, LRP, G);
     G.total_planes = (long long)A.batch * 3 * (A.nz - 2);
     static bool attr_done = false;      // per instantiation
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(k_diffuse_fused<NL, LRP>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        cudaError_t e = cudaFuncSetAttribute(k_diffuse_fused<NL, LRP, NX, NY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
-    k_diffuse_fused<NL, LRP><<<grid, G.nwarps * 32, G.smem_bytes, st>>>(A, G);
+    k_diffuse_fused<NL, LRP, NX, NY><<<grid, G.nwarps * 32, G.smem_bytes, st>>>(A, G);
     return cudaGetLastError();
+}
+
+template <int NL>
+inline cudaError_t fused_launch_nl(const FusedPlan &F, const FusedArgs &A, int grid, cudaStream_t st)
+{
+    if (F.fixed == 64) return fused_launch_t<NL, 32, 64, 64>(A, grid, st);
+    if (F.fixed == 32) return fused_launch_t<NL, 16, 32, 32>(A, grid, st);
+    if (F.lrp == 16) return fused_launch_t<NL, 16, 0, 0>(A, grid, st);
+    return fused_launch_t<NL, 32, 0, 0>(A, grid, st);
 }
 
 // Decide whether the fused kernel covers this lattice, and precompute its arguments.
@@ -371,6 +407,7 @@ inline void fused_configure(const KParams &P, FusedPlan &F)
     F.ok = false;
     if (P.nx % 2 || P.nx > 64 || P.nx < 4 || P.nz < 3 || (P.nx * P.ny) % 16 || P.n_sub < 1 || P.n_sub > 2 * F_MAXNL) return;
     F.lrp = P.nx <= 32 ? 16 : 32;
+    F.fixed = (P.nx == 64 && P.ny == 64) ? 64 : (P.nx == 32 && P.ny == 32) ? 32 : 0;
     FusedGeom G{};
     if (fused_smem(P.nx, P.ny, F_MAXNL, F.lrp, G) > 227 * 1024 || G.nwarps > 16) return;
     int dev = 0;
@@ -410,13 +447,13 @@ inline int launch_fused(FusedPlan &F, const Lattice &L, int cur, cudaStream_t st
         const long long total = (long long)A.batch * 3 * (A.nz - 2);
         const int grid = (int)std::max<long long>(1, std::min<long long>((long long)F.sms * per_sm, total / 2 + 1));
         cudaError_t e;
-        const int nl = F.pass_nl[ps];
-#define CA_FUSED_CASE(NLV) case NLV: e = (F.lrp == 16) ? fused_launch_t<NLV, 16>(A, G, grid, st) : fused_launch_t<NLV, 32>(A, G, grid, st); break;
-        switch (nl) {
-            CA_FUSED_CASE(1) CA_FUSED_CASE(2) CA_FUSED_CASE(3) CA_FUSED_CASE(4)
+        switch (F.pass_nl[ps]) {
+        case 1: e = fused_launch_nl<1>(F, A, grid, st); break;
+        case 2: e = fused_launch_nl<2>(F, A, grid, st); break;
+        case 3: e = fused_launch_nl<3>(F, A, grid, st); break;
+        case 4: e = fused_launch_nl<4>(F, A, grid, st); break;
         default: e = cudaErrorInvalidValue;
         }
-#undef CA_FUSED_CASE
         if (e != cudaSuccess) { *err = e; return ps; }
         cur ^= 1;
     }
