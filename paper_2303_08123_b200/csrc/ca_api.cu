@@ -64,6 +64,7 @@ struct ca_ctx {
     cudaStream_t stream;
     bool own_stream;
     int device;
+    int sms;
     int max_frac;
     int cur;                       // which ping-pong buffer holds the current fields
     long long step;                // host mirror of the device step counter
@@ -110,6 +111,13 @@ void drop_graphs(ca_ctx *c)
 
 inline unsigned int blocks_for(long long n, int threads) { return (unsigned int)((n + threads - 1) / threads); }
 
+// persistent grid of the sparse state scans: 8 CTAs of 8 warps per SM, never more than there are 4 KB trips
+unsigned int scan_grid(const ca_ctx *c)
+{
+    const long long trips = ((c->P.n * c->P.batch >> 4) + 255) >> 8;
+    return (unsigned int)std::max<long long>(1, std::min<long long>((long long)c->sms * 8, trips));
+}
+
 // Enqueue the kernels of ONE CA step (without irradiation) at device step *d_step + k, starting from
 // ping-pong buffer `cur`; returns the buffer holding the fields afterwards.   [D G15]
 int enqueue_step(ca_ctx *c, int cur, int k)
@@ -128,9 +136,9 @@ int enqueue_step(ca_ctx *c, int cur, int k)
         }
         c->launches += P.n_sub;
     }
-    k_cells<<<blocks_for(tot, 256), 256, 0, c->stream>>>(P, c->L, cur, c->d_step, k);                          // S2
-    k_div_detect<<<blocks_for(tot, 256), 256, 0, c->stream>>>(P, c->L, c->d_step, k, c->d_winners, c->d_nwin + k,
-                                                               c->Y.cap, c->d_err);                            // S3
+    const ScanArgs sa = { c->d_winners, c->d_nwin + k, c->Y.cap, c->d_err };
+    k_scan<0><<<scan_grid(c), 256, 0, c->stream>>>(P, c->L, cur, c->d_step, k, sa);                            // S2
+    k_scan<1><<<scan_grid(c), 256, 0, c->stream>>>(P, c->L, cur, c->d_step, k, sa);                            // S3 detect
     k_div_apply<<<64, 128, 0, c->stream>>>(P, c->L, c->d_step, k, c->d_winners, c->d_nwin + k, c->Y.cap);
     c->launches += 3;
     return cur;
@@ -312,6 +320,7 @@ int ca_create(ca_ctx **out, int batch, int nx, int ny, int nz, const ca_params *
         c->own_stream = true;
     }
     c->device = dev;
+    c->sms = prop.multiProcessorCount;
     c->max_frac = max_frac;
     c->cur = 0; c->step = 0; c->seeded = false;
     c->fire.assign((size_t)batch * max_frac, 0); c->dose.assign((size_t)batch * max_frac, 0.0f); c->nfrac.assign(batch, 0);
@@ -523,9 +532,11 @@ int ca_stage(ca_ctx *c, int stage, int arg)
         }
         else for (int m = 0; m < P.n_sub; ++m) { k_diffuse_sub<<<blocks_for(tot, 256), 256, 0, c->stream>>>(P, c->L, c->cur); c->cur ^= 1; c->launches += 1; }
         break;
-    case 2: k_cells<<<blocks_for(tot, 256), 256, 0, c->stream>>>(P, c->L, c->cur, c->d_step, 0); c->launches += 1; break;
+    case 2: { const ScanArgs sa = { c->d_winners, c->d_nwin, c->Y.cap, c->d_err };
+              k_scan<0><<<scan_grid(c), 256, 0, c->stream>>>(P, c->L, c->cur, c->d_step, 0, sa); c->launches += 1; break; }
     case 3:
-        k_div_detect<<<blocks_for(tot, 256), 256, 0, c->stream>>>(P, c->L, c->d_step, 0, c->d_winners, c->d_nwin, c->Y.cap, c->d_err);
+        { const ScanArgs sa = { c->d_winners, c->d_nwin, c->Y.cap, c->d_err };
+          k_scan<1><<<scan_grid(c), 256, 0, c->stream>>>(P, c->L, c->cur, c->d_step, 0, sa); }
         k_div_apply<<<64, 128, 0, c->stream>>>(P, c->L, c->d_step, 0, c->d_winners, c->d_nwin, c->Y.cap);
         enqueue_advance(c, 0);
         c->launches += 2;

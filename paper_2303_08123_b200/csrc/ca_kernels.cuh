@@ -155,22 +155,117 @@ __device__ __forceinline__ void cell_update(const KParams &P, uint32_t &st, uint
     }
 }
 
-__global__ void k_cells(KParams P, Lattice L, int cur, const long long *__restrict__ d_step, int k)
+// S2 for one occupied site
+__device__ __forceinline__ void cells_site(const KParams &P, const Lattice &L, int cur, long long gi, uint32_t st, uint32_t step)
 {
-    const long long gi = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (gi >= P.n * P.batch) return;
-    uint32_t st = L.state[gi];
-    const int kind = st & 7;
-    if (kind == CA_EMPTY || kind == CA_WALL) return;
     const int b = (int)(gi / P.n);
     const uint32_t i = (uint32_t)(gi - (long long)b * P.n);
-    const uint32_t step = (uint32_t)(*d_step + k);
     uint32_t ck = L.clock[gi], dm = L.damage[gi];
     const uint32_t st0 = st, ck0 = ck, dm0 = dm;
     cell_update(P, st, ck, dm, L.f[cur][0][gi], L.f[cur][1][gi], L.f[cur][2][gi], i, step, P.sim_id_base + (uint32_t)b);
     if (st != st0) L.state[gi] = (uint8_t)st;
     if (ck != ck0) L.clock[gi] = (uint16_t)ck;
     if (dm != dm0) L.damage[gi] = (uint16_t)dm;
+}
+
+// Sparse scan of the state array shared by S2 and S3.  A persistent grid walks the flat array in 16-byte
+// chunks per lane (4 KB per CTA and trip, the next trip prefetched).  At configs[1] ~99 % of the chunks hold no
+// cell and cost a few compares; when a CTA finds sites of interest it compacts them into a shared-memory
+// queue and works them off one site per thread, so a dense tumour core is spread over all 256 threads
+// instead of serialising inside the lanes that happened to load it.
+//   MODE 0: S2, sites holding a cell (kind not EMPTY / WALL);   MODE 1: S3, READY parents.
+template <int MODE>
+__device__ __forceinline__ uint32_t scan_word_mask(uint32_t w)
+{
+    uint32_t m = 0;
+    if (MODE == 0) {
+        if ((((w & 0x07070707u) + 0x01010101u) & 0x06060606u) == 0u) return 0u;   // every byte EMPTY or WALL
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const uint32_t kind = (w >> (8 * r)) & 7u;
+            m |= (kind != CA_EMPTY && kind != CA_WALL) ? (1u << r) : 0u;
+        }
+    } else {
+        if ((w & 0x20202020u) == 0u) return 0u;                                    // no READY byte
+#pragma unroll
+        for (int r = 0; r < 4; ++r) m |= is_parent((w >> (8 * r)) & 0xFFu) ? (1u << r) : 0u;
+    }
+    return m;
+}
+
+struct ScanArgs {                 // S3 only
+    unsigned long long *winners;
+    unsigned int *nwin;
+    unsigned int cap;
+    int *err;
+};
+
+__device__ __forceinline__ void detect_site(const KParams &P, const Lattice &L, long long gi, uint32_t step,
+                                            unsigned long long *__restrict__ winners, unsigned int *__restrict__ nwin,
+                                            unsigned int cap, int *__restrict__ err);
+
+template <int MODE>
+__global__ void __launch_bounds__(256) k_scan(KParams P, Lattice L, int cur, const long long *__restrict__ d_step, int k, ScanArgs S)
+{
+    // one trip of a CTA = 256 lanes x 16 bytes = 4 KB of the state array (one 64x64 plane at configs[1])
+    __shared__ uint32_t queue[4096];
+    __shared__ uint32_t qn;
+    const long long tot = P.n * P.batch;
+    const long long nchunk = tot >> 4;
+    const uint32_t step = (uint32_t)(*d_step + k);
+    const int lane = threadIdx.x & 31;
+    const long long ntrip = (nchunk + 255) >> 8;
+    if (threadIdx.x == 0) qn = 0;
+    __syncthreads();
+    long long trip = blockIdx.x;
+    uint4 w = make_uint4(0u, 0u, 0u, 0u);
+    if (trip < ntrip && trip * 256 + threadIdx.x < nchunk) w = reinterpret_cast<const uint4 *>(L.state)[trip * 256 + threadIdx.x];
+    for (; trip < ntrip; trip += gridDim.x) {
+        const uint32_t ws[4] = { w.x, w.y, w.z, w.w };
+        const long long nxt = trip + gridDim.x;                                     // prefetch the next trip before working on this one
+        w = make_uint4(0u, 0u, 0u, 0u);
+        if (nxt < ntrip && nxt * 256 + threadIdx.x < nchunk) w = reinterpret_cast<const uint4 *>(L.state)[nxt * 256 + threadIdx.x];
+        uint32_t m = 0;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) m |= scan_word_mask<MODE>(ws[q]) << (4 * q);
+        if (!__syncthreads_or(m != 0u)) continue;                                    // nothing of interest in these 4 KB
+        // compact the sites of interest of the whole CTA into the queue (order is irrelevant to the result)
+        const uint32_t cnt = __popc(m);
+        uint32_t pre = cnt;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, pre, o);
+            if (lane >= o) pre += v;
+        }
+        uint32_t base = 0;
+        if (lane == 31 && pre) base = atomicAdd(&qn, pre);
+        base = __shfl_sync(0xFFFFFFFFu, base, 31);
+        uint32_t pos = base + pre - cnt;
+        uint32_t mm = m;
+        while (mm) {
+            const int bit = __ffs(mm) - 1;
+            mm &= mm - 1;
+            const uint32_t st = (ws[bit >> 2] >> (8 * (bit & 3))) & 0xFFu;
+            queue[pos++] = (uint32_t)(threadIdx.x * 16 + bit) | (st << 16);
+        }
+        __syncthreads();
+        const uint32_t total = qn;
+        for (uint32_t r = threadIdx.x; r < total; r += 256) {
+            const uint32_t e = queue[r];
+            const long long gi = trip * 4096 + (e & 0xFFFFu);
+            if (MODE == 0) cells_site(P, L, cur, gi, e >> 16, step);
+            else detect_site(P, L, gi, step, S.winners, S.nwin, S.cap, S.err);
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) qn = 0;                                                // ordered before the next use by the __syncthreads_or above
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0)                                       // ragged tail of the flat array (tot % 16 sites)
+        for (long long gi = nchunk * 16; gi < tot; ++gi) {
+            const uint32_t st = L.state[gi];
+            const uint32_t kind = st & 7u;
+            if (MODE == 0) { if (kind != CA_EMPTY && kind != CA_WALL) cells_site(P, L, cur, gi, st, step); }
+            else if (is_parent(st)) detect_site(P, L, gi, step, S.winners, S.nwin, S.cap, S.err);
+        }
 }
 
 // ---------------------------------------------------------------------- S3 --
@@ -193,17 +288,13 @@ __device__ __forceinline__ int choose_dir(const KParams &P, const uint8_t *__res
     return best;
 }
 
-__global__ void k_div_detect(KParams P, Lattice L, const long long *__restrict__ d_step, int k,
-                             unsigned long long *__restrict__ winners, unsigned int *__restrict__ nwin,
-                             unsigned int cap, int *__restrict__ err)
+__device__ __forceinline__ void detect_site(const KParams &P, const Lattice &L, long long gi, uint32_t step,
+                                            unsigned long long *__restrict__ winners, unsigned int *__restrict__ nwin,
+                                            unsigned int cap, int *__restrict__ err)
 {
-    const long long gi = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (gi >= P.n * P.batch) return;
-    if (!is_parent(L.state[gi])) return;
     const int b = (int)(gi / P.n);
     const uint32_t p = (uint32_t)(gi - (long long)b * P.n);
     const uint8_t *sb = L.state + (long long)b * P.n;
-    const uint32_t step = (uint32_t)(*d_step + k);
     const uint32_t sid = P.sim_id_base + (uint32_t)b;
     const int off[6] = { -1, 1, -P.nx, P.nx, -P.nx * P.ny, P.nx * P.ny };
     const int dir = choose_dir(P, sb, p, step, sid, off);
