@@ -22,7 +22,7 @@ thread_local std::string g_create_error;
 size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 
 struct Layout {
-    size_t field[2][3], state, clock, damage, winners, nwin, step, err, counts, fitness, fire, dose, nfrac, stage, total;
+    size_t field[2][3], state, clock, damage, occ, winners, nwin, step, err, counts, fitness, fire, dose, nfrac, stage, total;
     unsigned int cap;
 };
 
@@ -36,6 +36,7 @@ Layout make_layout(int batch, long long n, int max_frac)
     Y.state = o;   o = align_up(o + tot);
     Y.clock = o;   o = align_up(o + tot * 2);
     Y.damage = o;  o = align_up(o + tot * 2);
+    Y.occ = o;     o = align_up(o + (tot / 256 + 64) * 4);   // occupancy map of the S2/S3 fast path
     size_t cap = std::max<size_t>(65536, tot / 8);
     if (cap > (1u << 28)) cap = 1u << 28;
     Y.cap = (unsigned int)cap;
@@ -77,6 +78,10 @@ struct ca_ctx {
     int *d_fire; float *d_dose; int *d_nfrac;
     unsigned long long *d_winners; unsigned int *d_nwin; long long *d_step; int *d_err; int *d_counts; float *d_fitness;
     uint8_t *d_stage;
+    uint32_t *d_occ;
+    bool mapped_ok;               // simulations are whole multiples of 256 sites: clustered S2+S3 kernel usable
+    int cell_path;                 // option: 1 = clustered S2+S3 kernel when usable, 0 = generic scan kernels
+    int cs;                        // CTAs per simulation (cluster size) of the clustered kernel
     // options
     int graph_steps;
     int fused;
@@ -118,23 +123,51 @@ unsigned int scan_grid(const ca_ctx *c)
     return (unsigned int)std::max<long long>(1, std::min<long long>((long long)c->sms * 8, trips));
 }
 
+// S2 and/or S3 through the occupancy map: one cluster of c->cs CTAs per simulation
+void enqueue_cells_divide(ca_ctx *c, int cur, int k, int phases, bool have_map)
+{
+    const KParams &P = c->P;
+    const long long tot = P.n * P.batch;
+    if (!have_map) {
+        k_occ_map<<<blocks_for(tot / 8, 256), 256, 0, c->stream>>>(c->L.state, tot, c->d_occ);
+        c->launches += 1;
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned int)(P.batch * c->cs));
+    cfg.blockDim = dim3(CD_THREADS);
+    cfg.stream = c->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = (unsigned int)c->cs; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, k_cells_divide, P, c->L, cur, (const long long *)c->d_step, k, (const uint32_t *)c->d_occ, c->cs, phases, c->d_err);
+    c->launches += 1;
+}
+
 // Enqueue the kernels of ONE CA step (without irradiation) at device step *d_step + k, starting from
 // ping-pong buffer `cur`; returns the buffer holding the fields afterwards.   [D G15]
 int enqueue_step(ca_ctx *c, int cur, int k)
 {
     const KParams &P = c->P;
     const long long tot = P.n * P.batch;
+    const bool mapped = c->mapped_ok && c->cell_path;
+    bool have_map = false;
     if (c->fused && fused_supported(c->fplan)) {
         cudaError_t fe;
-        const int np = launch_fused(c->fplan, c->L, cur, c->stream, &fe);   // S1: all n_sub sub-steps, one pass over HBM (two if n_sub > 4)
+        const int np = launch_fused(c->fplan, c->L, cur, mapped ? c->d_occ : nullptr, c->stream, &fe);   // S1: all n_sub sub-steps, one pass over HBM (two if n_sub > 4)
         if (np & 1) cur ^= 1;
         c->launches += np;
+        have_map = mapped && c->fplan.fixed != 0;
     } else {
         for (int m = 0; m < P.n_sub; ++m) {                                // S1, one launch per sub-step
             k_diffuse_sub<<<blocks_for(tot, 256), 256, 0, c->stream>>>(P, c->L, cur);
             cur ^= 1;
         }
         c->launches += P.n_sub;
+    }
+    if (mapped) {
+        enqueue_cells_divide(c, cur, k, 3, have_map);                       // S2 + S3 in one clustered launch
+        return cur;
     }
     const ScanArgs sa = { c->d_winners, c->d_nwin + k, c->Y.cap, c->d_err };
     k_scan<0><<<scan_grid(c), 256, 0, c->stream>>>(P, c->L, cur, c->d_step, k, sa);                            // S2
@@ -312,6 +345,7 @@ int ca_create(ca_ctx **out, int batch, int nx, int ny, int nz, const ca_params *
     c->d_dose = (float *)(c->ws + c->Y.dose);
     c->d_nfrac = (int *)(c->ws + c->Y.nfrac);
     c->d_stage = c->ws + c->Y.stage;
+    c->d_occ = (uint32_t *)(c->ws + c->Y.occ);
     c->stream = (cudaStream_t)stream;
     c->own_stream = false;
     if (!c->stream) {                     // the legacy default stream cannot be captured into CUDA graphs
@@ -325,6 +359,13 @@ int ca_create(ca_ctx **out, int batch, int nx, int ny, int nz, const ca_params *
     c->cur = 0; c->step = 0; c->seeded = false;
     c->fire.assign((size_t)batch * max_frac, 0); c->dose.assign((size_t)batch * max_frac, 0.0f); c->nfrac.assign(batch, 0);
     c->graph_steps = 20; c->fused = 1;
+    c->mapped_ok = (n % 256 == 0) && n < (1ll << 29);
+    c->cell_path = 1;
+    {
+        int cs = 1;
+        while (cs < 8 && (long long)batch * cs * 2 <= 2ll * c->sms && (n >> 8) / 128 >= 2 * cs) cs *= 2;
+        c->cs = cs;
+    }
     c->graph[0] = c->graph[1] = nullptr; c->graph_len[0] = c->graph_len[1] = 0; c->graph_nodes = 0; c->launches = 0;
     // zero the small control blocks (protocol tables, counters)
     e = cudaMemsetAsync(c->ws + c->Y.winners, 0, c->Y.total - c->Y.winners, c->stream);
@@ -526,15 +567,19 @@ int ca_stage(ca_ctx *c, int stage, int arg)
     case 1:
         if (c->fused && fused_supported(c->fplan)) {
             cudaError_t fe;
-            const int np = launch_fused(c->fplan, c->L, c->cur, c->stream, &fe);
+            const int np = launch_fused(c->fplan, c->L, c->cur, nullptr, c->stream, &fe);
             if (np & 1) c->cur ^= 1;
             c->launches += np;
         }
         else for (int m = 0; m < P.n_sub; ++m) { k_diffuse_sub<<<blocks_for(tot, 256), 256, 0, c->stream>>>(P, c->L, c->cur); c->cur ^= 1; c->launches += 1; }
         break;
-    case 2: { const ScanArgs sa = { c->d_winners, c->d_nwin, c->Y.cap, c->d_err };
-              k_scan<0><<<scan_grid(c), 256, 0, c->stream>>>(P, c->L, c->cur, c->d_step, 0, sa); c->launches += 1; break; }
+    case 2:
+        if (c->mapped_ok && c->cell_path) { enqueue_cells_divide(c, c->cur, 0, 1, false); break; }
+        { const ScanArgs sa = { c->d_winners, c->d_nwin, c->Y.cap, c->d_err };
+          k_scan<0><<<scan_grid(c), 256, 0, c->stream>>>(P, c->L, c->cur, c->d_step, 0, sa); c->launches += 1; }
+        break;
     case 3:
+        if (c->mapped_ok && c->cell_path) { enqueue_cells_divide(c, c->cur, 0, 2, false); break; }
         { const ScanArgs sa = { c->d_winners, c->d_nwin, c->Y.cap, c->d_err };
           k_scan<1><<<scan_grid(c), 256, 0, c->stream>>>(P, c->L, c->cur, c->d_step, 0, sa); }
         k_div_apply<<<64, 128, 0, c->stream>>>(P, c->L, c->d_step, 0, c->d_winners, c->d_nwin, c->Y.cap);
@@ -558,6 +603,7 @@ int ca_set_option(ca_ctx *c, const char *name, int value)
         c->graph_steps = value; drop_graphs(c); return CA_OK;
     }
     if (!std::strcmp(name, "fused")) { c->fused = value ? 1 : 0; drop_graphs(c); return CA_OK; }
+    if (!std::strcmp(name, "cell_path")) { c->cell_path = value ? 1 : 0; drop_graphs(c); return CA_OK; }
     return fail(c, CA_EINVAL, std::string("unknown option ") + name);
 }
 

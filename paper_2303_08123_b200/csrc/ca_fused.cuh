@@ -45,6 +45,7 @@ struct FusedArgs {
     float lut[3][32];          // source term by (state & 31): rate[s][mode] if kind in 1..4 else 0  [D G4]
     int always_slow[3];        // 1: the clamp cannot be proven idle for this lambda -> always take the full path
     float zero;                // 0.0f, opaque to ptxas (see Fused::level)
+    uint32_t *occ;             // occupancy map for S2/S3 (one bit per 8 state bytes), written by the fixed-size kernels; may be NULL
 };
 
 // ---- packed f32x2 arithmetic (Blackwell FADD2/FMUL2/FFMA2); .rn, no ftz: identical to two scalar ops ----
@@ -112,6 +113,7 @@ struct FusedCtx {
     u64 zero2;                 // (0, 0) that ptxas cannot see through
     uint32_t rowmask;          // bit j: row y0+j exists and this lane's x pair is inside the lattice
     bool strip_ok;
+    uint32_t *occ_row;         // species 0 only: occupancy words of this warp's strip, indexed by plane (else NULL)
 };
 
 // NX = NY = 0: lattice dims at run time (any even nx <= 2*LRP); otherwise compile-time dims, all address math folds
@@ -128,10 +130,9 @@ struct Fused {
     static __device__ __forceinline__ uint32_t exl(const FusedCtx &c) { return FIXED ? EXL : c.ex_lvl; }
     static __device__ __forceinline__ bool row(const FusedCtx &c, int j) { return FULL ? true : ((c.rowmask >> j) & 1u) != 0u; }
 
-    // one sub-step of [D S1] for this lane's 2 x 4 points; C = centre plane, M/P = planes z-1/z+1 (same level)
-    template <bool SLOW>
+    // the diffusion part of one sub-step of [D S1] for this lane's 2 x 4 points; C = centre plane, M/P = planes z-1/z+1
     static __device__ __forceinline__ void level(const u64 (&M)[F_PY], const u64 (&C)[F_PY], const u64 (&P)[F_PY], u64 (&N)[F_PY],
-                                                 u64 up, u64 dn, const u64 (&lam2)[F_PY], const u64 (&r2)[F_PY], const u64 zero2)
+                                                 u64 up, u64 dn, const u64 (&lam2)[F_PY], const u64 zero2)
     {
         const u64 six2 = pk(6.0f, 6.0f);
 #pragma unroll
@@ -147,14 +148,7 @@ struct Fused {
             // 6*c must be rounded on its own [D S1].  ptxas contracts mul.rn.f32x2 + sub.rn.f32x2 into one FFMA2 (seen in SASS,
             // CUDA 12.9), so the product is formed as fma(6, c, 0) with a zero the compiler cannot fold: same value, same pipe cost.
             const u64 lap = sub2(s6, fma2(six2, C[j], zero2));
-            u64 v = fma2(lam2[j], lap, C[j]);
-            if (SLOW) {
-                v = add2(v, r2[j]);
-                float a, b;
-                upk(v, a, b);
-                v = pk(fmaxf(a, 0.0f), fmaxf(b, 0.0f));
-            }
-            N[j] = v;
+            N[j] = fma2(lam2[j], lap, C[j]);                                 // the source term and the clamp follow in levels()
         }
     }
 
@@ -188,21 +182,19 @@ struct Fused {
                 const uint32_t el = exl(c);
                 const u64 up = lds64(exr + (uint32_t)(K - 1) * el + (el / 2 - GRP));     // bottom row of the strip above
                 const u64 dn = lds64(exr + (uint32_t)(K - 1) * el + GRP);                // top row of the strip below
-                u64 r2[F_PY];
                 u64 nloc[F_PY];
                 u64 (&N)[F_PY] = *(K < NL ? &h[KO][sc] : &nloc);
-                if (((c.flags | c.slowmask) >> K) & 1u) {
+                level(h[K - 1][sm], h[K - 1][sc], h[K - 1][sp], N, up, dn, c.lam2, c.zero2);
+                if (((c.flags | c.slowmask) >> K) & 1u) {                  // cells in this strip: source term and clamp
                     const uint32_t s = c.st_lane + ((q - (uint32_t)K) & (F_SRING - 1)) * (uint32_t)nxny(c);
 #pragma unroll
                     for (int j = 0; j < F_PY; ++j) {
                         const uint32_t w = row(c, j) ? lds16(s + (uint32_t)(j * nx(c))) : 0u;
-                        r2[j] = pk(lds32f(c.lut + (w & 31u) * 4u), lds32f(c.lut + ((w >> 8) & 31u) * 4u));
+                        const u64 v = add2(N[j], pk(lds32f(c.lut + (w & 31u) * 4u), lds32f(c.lut + ((w >> 8) & 31u) * 4u)));
+                        float a, b;
+                        upk(v, a, b);
+                        N[j] = pk(fmaxf(a, 0.0f), fmaxf(b, 0.0f));
                     }
-                    level<true>(h[K - 1][sm], h[K - 1][sc], h[K - 1][sp], N, up, dn, c.lam2, r2, c.zero2);
-                } else {
-#pragma unroll
-                    for (int j = 0; j < F_PY; ++j) r2[j] = 0ull;
-                    level<false>(h[K - 1][sm], h[K - 1][sc], h[K - 1][sp], N, up, dn, c.lam2, r2, c.zero2);
                 }
                 if constexpr (K < NL) {
                     sts64(exw + (uint32_t)K * el, N[0]);
@@ -256,7 +248,12 @@ struct Fused {
             const u64 w = c.strip_ok ? lds64(c.st_strip + (q & (F_SRING - 1)) * (uint32_t)nxny(c)) : 0ull;
             any = (((w & 0x0707070707070707ull) + 0x0101010101010101ull) & 0x0606060606060606ull) != 0ull;
         }
-        c.flags = (c.flags << 1) | (__any_sync(0xFFFFFFFFu, any) ? 1u : 0u);
+        const uint32_t ballot = __ballot_sync(0xFFFFFFFFu, any);
+        c.flags = (c.flags << 1) | (ballot ? 1u : 0u);
+        if constexpr (FIXED) {                                              // the same vote is the S2/S3 occupancy map: strip = 256 contiguous bytes
+            if ((threadIdx.x & 31) == 0 && c.occ_row != nullptr && (STEADY || (t >= c.ld_lo && t < c.ld_hi)))
+                c.occ_row[(size_t)t * (NX * NY / 256)] = ballot;
+        }
         // ---- levels 1..NL: level k computes plane t-k from level k-1
         levels<PH, 1, STEADY>(t, q, exr, exw, h, c);
         __syncthreads();
@@ -330,6 +327,7 @@ __global__ void __launch_bounds__(512, 1) k_diffuse_fused(const FusedArgs A, con
         c.st_lo = 2 * NL; c.st_hi = min(A.nz, c.zb + NL) - c.t0;              // za+NL <= t < min(nz, zb+NL)
         c.flags = 0; c.slowmask = A.always_slow[sp] ? 0xFFFFFFFFu : 0u;
         c.lut = base + Gm.off_lut + (uint32_t)sp * 128u;
+        c.occ_row = (sp == 0 && A.occ != nullptr && NX != 0) ? A.occ + (size_t)b * (size_t)(c.nxny / 256) * (size_t)A.nz + warp : nullptr;
         const float lam = A.lam[sp];
 #pragma unroll
         for (int j = 0; j < F_PY; ++j) {
@@ -337,9 +335,10 @@ __global__ void __launch_bounds__(512, 1) k_diffuse_fused(const FusedArgs A, con
             const bool rowin = y > 0 && y < nyr - 1;                           // y walls and rows outside the lattice: lambda = 0
             c.lam2[j] = pk(rowin && x0 > 0 && x0 < nxr - 1 ? lam : 0.0f, rowin && x0 + 1 < nxr - 1 ? lam : 0.0f);
         }
+        const int i0 = ((c.ld_lo - c.t0) / 3) * 3;                           // iterations before the first loaded plane have nothing to do
         if (tid == 0)
-            for (int i = 0; i < F_RING - 1 && i < c.nsteps; ++i) F::issue(c, i, i);
-        for (int i = 0; i < c.nsteps; i += 3) {
+            for (int i = i0; i < i0 + F_RING - 1 && i < c.nsteps; ++i) F::issue(c, i, i - i0);
+        for (int i = i0; i < c.nsteps; i += 3) {
             if (i >= c.st_lo && i + 3 <= c.st_hi) {
                 F::template step<0, true>(i, h, c);
                 F::template step<1, true>(i + 1, h, c);
@@ -433,13 +432,14 @@ inline void fused_configure(const KParams &P, FusedPlan &F)
 inline bool fused_supported(const FusedPlan &F) { return F.ok; }
 
 // Enqueue all n_sub sub-steps starting from ping-pong buffer `cur`; returns the number of passes (= buffer flips).
-inline int launch_fused(FusedPlan &F, const Lattice &L, int cur, cudaStream_t st, cudaError_t *err)
+inline int launch_fused(FusedPlan &F, const Lattice &L, int cur, uint32_t *occ, cudaStream_t st, cudaError_t *err)
 {
     *err = cudaSuccess;
     for (int ps = 0; ps < F.npass; ++ps) {
         FusedArgs A = F.args;
         for (int s = 0; s < 3; ++s) { A.src[s] = L.f[cur][s]; A.dst[s] = L.f[cur ^ 1][s]; }
         A.state = L.state;
+        A.occ = (F.fixed && ps == F.npass - 1) ? occ : nullptr;          // the state does not change between passes: write the map once
         FusedGeom G{};
         // CTAs per SM: the 512-thread (nx > 32) kernel fills an SM; smaller lattices use several CTAs per SM
         fused_smem(A.nx, A.ny, F.pass_nl[ps], F.lrp, G);

@@ -281,11 +281,32 @@ __device__ __forceinline__ int choose_dir(const KParams &P, const uint8_t *__res
     uint32_t bk = 0;
 #pragma unroll
     for (int d = 0; d < 6; ++d) {
-        if (sb[(int)p + off[d]] != CA_EMPTY) continue;                     // WALL != EMPTY: targets are interior
-        const uint32_t kk = rnd(P, p, step, sid, P_DIR, (uint32_t)d);
+        if (__ldcg(sb + ((int)p + off[d])) != CA_EMPTY) continue;          // WALL != EMPTY: targets are interior.  L2 loads: the
+        const uint32_t kk = rnd(P, p, step, sid, P_DIR, (uint32_t)d);      // neighbour may have been written by another SM in S2
         if (best < 0 || kk < bk) { best = d; bk = kk; }                    // ties -> lower dir
     }
     return best;
+}
+
+// Does READY parent p (site index inside its simulation, state array sb) win a target on this step?
+// Returns the direction of its daughter, or -1 (blocked, or lost the claim: untouched, retries next step).
+__device__ __forceinline__ int detect_decide(const KParams &P, const uint8_t *__restrict__ sb, uint32_t p, uint32_t step, uint32_t sid)
+{
+    const int off[6] = { -1, 1, -P.nx, P.nx, -P.nx * P.ny, P.nx * P.ny };
+    const int dir = choose_dir(P, sb, p, step, sid, off);
+    if (dir < 0) return -1;                                                // blocked: stays READY, retries
+    const uint32_t e = (uint32_t)((int)p + off[dir]);
+    const uint32_t mykey = rnd(P, p, step, sid, P_CLAIM);
+#pragma unroll 1
+    for (int d = 0; d < 6; ++d) {                                          // competitors = other neighbours of e
+        const uint32_t q = (uint32_t)((int)e + off[d]);
+        if (q == p || !is_parent(__ldcg(sb + q))) continue;
+        const int dq = choose_dir(P, sb, q, step, sid, off);
+        if (dq < 0 || (uint32_t)((int)q + off[dq]) != e) continue;
+        const uint32_t qk = rnd(P, q, step, sid, P_CLAIM);
+        if (qk < mykey || (qk == mykey && q < p)) return -1;
+    }
+    return dir;
 }
 
 __device__ __forceinline__ void detect_site(const KParams &P, const Lattice &L, long long gi, uint32_t step,
@@ -294,25 +315,27 @@ __device__ __forceinline__ void detect_site(const KParams &P, const Lattice &L, 
 {
     const int b = (int)(gi / P.n);
     const uint32_t p = (uint32_t)(gi - (long long)b * P.n);
-    const uint8_t *sb = L.state + (long long)b * P.n;
-    const uint32_t sid = P.sim_id_base + (uint32_t)b;
-    const int off[6] = { -1, 1, -P.nx, P.nx, -P.nx * P.ny, P.nx * P.ny };
-    const int dir = choose_dir(P, sb, p, step, sid, off);
-    if (dir < 0) return;                                                   // blocked: stays READY, retries
-    const uint32_t e = (uint32_t)((int)p + off[dir]);
-    const uint32_t mykey = rnd(P, p, step, sid, P_CLAIM);
-#pragma unroll 1
-    for (int d = 0; d < 6; ++d) {                                          // competitors = other neighbours of e
-        const uint32_t q = (uint32_t)((int)e + off[d]);
-        if (q == p || !is_parent(sb[q])) continue;
-        const int dq = choose_dir(P, sb, q, step, sid, off);
-        if (dq < 0 || (uint32_t)((int)q + off[dq]) != e) continue;
-        const uint32_t qk = rnd(P, q, step, sid, P_CLAIM);
-        if (qk < mykey || (qk == mykey && q < p)) return;                  // lost: untouched, retries next step
-    }
+    const int dir = detect_decide(P, L.state + (long long)b * P.n, p, step, P.sim_id_base + (uint32_t)b);
+    if (dir < 0) return;
     const unsigned int slot = atomicAdd(nwin, 1u);                         // list order is irrelevant to the result
     if (slot >= cap) { *err = CA_EOVERFLOW; return; }
     winners[slot] = ((unsigned long long)gi << 3) | (unsigned long long)dir;
+}
+
+// [D S3 step 4] write one winner: parent and daughter both restart in G1 with fresh clocks
+__device__ __forceinline__ void apply_winner(const KParams &P, const Lattice &L, int b, uint32_t p, int dir, uint32_t step)
+{
+    const int off[6] = { -1, 1, -P.nx, P.nx, -P.nx * P.ny, P.nx * P.ny };
+    const long long gp = (long long)b * P.n + p;
+    const uint32_t e = (uint32_t)((int)p + off[dir]);
+    const long long ge = gp + off[dir];
+    const uint32_t sid = P.sim_id_base + (uint32_t)b;
+    const uint32_t keep = L.state[gp] & (0x18u | CA_DOOMED);              // mode and DOOMED carried to both [D G10]
+    L.state[gp] = (uint8_t)(CA_G1 | keep);
+    L.clock[gp] = draw_clock(P, CA_G1, p, step, sid, P_PARENT_CLOCK);
+    L.state[ge] = (uint8_t)(CA_G1 | keep);
+    L.clock[ge] = draw_clock(P, CA_G1, e, step, sid, P_DAUGHTER_CLOCK);
+    L.damage[ge] = L.damage[gp];
 }
 
 __global__ void k_div_apply(KParams P, Lattice L, const long long *__restrict__ d_step, int k,
@@ -322,22 +345,139 @@ __global__ void k_div_apply(KParams P, Lattice L, const long long *__restrict__ 
     unsigned int n = *nwin;
     if (n > cap) n = cap;
     const uint32_t step = (uint32_t)(*d_step + k);
-    const int off[6] = { -1, 1, -P.nx, P.nx, -P.nx * P.ny, P.nx * P.ny };
     for (unsigned int w = blockIdx.x * blockDim.x + threadIdx.x; w < n; w += gridDim.x * blockDim.x) {
         const unsigned long long ent = winners[w];
         const long long gp = (long long)(ent >> 3);
-        const int dir = (int)(ent & 7ull);
         const int b = (int)(gp / P.n);
-        const uint32_t p = (uint32_t)(gp - (long long)b * P.n);
-        const uint32_t e = (uint32_t)((int)p + off[dir]);
-        const long long ge = gp + off[dir];
-        const uint32_t sid = P.sim_id_base + (uint32_t)b;
-        const uint32_t keep = L.state[gp] & (0x18u | CA_DOOMED);          // mode and DOOMED carried to both [D G10]
-        L.state[gp] = (uint8_t)(CA_G1 | keep);
-        L.clock[gp] = draw_clock(P, CA_G1, p, step, sid, P_PARENT_CLOCK);
-        L.state[ge] = (uint8_t)(CA_G1 | keep);
-        L.clock[ge] = draw_clock(P, CA_G1, e, step, sid, P_DAUGHTER_CLOCK);
-        L.damage[ge] = L.damage[gp];
+        apply_winner(P, L, b, (uint32_t)(gp - (long long)b * P.n), (int)(ent & 7ull), step);
+    }
+}
+
+// ------------------------------------------------------------ S2 + S3 fused --
+// Fast path for lattices whose simulations are whole multiples of 256 sites.  It works from an occupancy
+// map -- one bit per 8 consecutive state bytes, set when a byte holds kind 1..6 -- that the fused diffusion
+// kernel produces for free while the state planes pass through its shared memory (k_occ_map builds it
+// when that kernel is not in use).  The map is taken before S2 of the same step; S2 never fills an EMPTY
+// site and S3's births are applied last, so it covers every site S2 and S3 have to look at.
+//
+// One thread-block cluster per simulation does S2, S3-detect and S3-apply in ONE launch: S3 needs every
+// S2 result of the simulation, which a cluster barrier provides (simulations never interact), and winners
+// stay in shared memory.  Work is taken from the map, never from a sweep over the lattice.
+__global__ void __launch_bounds__(256) k_occ_map(const uint8_t *__restrict__ state, long long tot, uint32_t *__restrict__ occ)
+{
+    const long long c8 = (long long)blockIdx.x * blockDim.x + threadIdx.x;          // 8-byte chunk index; tot % 256 == 0
+    bool any = false;
+    if (c8 * 8 < tot) {
+        const unsigned long long w = reinterpret_cast<const unsigned long long *>(state)[c8];
+        any = (((w & 0x0707070707070707ull) + 0x0101010101010101ull) & 0x0606060606060606ull) != 0ull;
+    }
+    const uint32_t ballot = __ballot_sync(0xFFFFFFFFu, any);
+    if ((threadIdx.x & 31) == 0 && c8 * 8 < tot) occ[c8 >> 5] = ballot;
+}
+
+constexpr int CD_THREADS = 512;
+constexpr int CD_WCAP = 4096;     // map words examined per round
+constexpr int CD_GROUP = 16;      // non-empty map words expanded at a time: at most 16 * 256 = 4096 sites
+constexpr int CD_QCAP = CD_GROUP * 256;
+constexpr int CD_WINCAP = 1024;   // winners per CTA and step
+
+struct CDShared {
+    uint32_t W[CD_WCAP];          // indices of the non-empty map words of this round
+    uint32_t Q[CD_QCAP];          // sites to work on (index inside the simulation)
+    uint8_t Qst[CD_QCAP];         // their state bytes
+    uint32_t win[CD_WINCAP];      // winners: parent site << 3 | direction
+    uint32_t nW, nQ, nwin;
+};
+
+__device__ __forceinline__ void cluster_sync_all()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+
+// MODE 0: S2 on every cell of simulation b;  MODE 1: S3 detect on every READY parent.
+// CTA `rank` of `cs` takes the 128-word tiles rank, rank + cs, ... of the simulation's map.
+template <int MODE>
+__device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int cur, int b, int rank, int cs, uint32_t step,
+                                        const uint32_t *__restrict__ occ_b, uint32_t nblk, CDShared &sh, int *__restrict__ err)
+{
+    const int tid = threadIdx.x;
+    const long long sbase = (long long)b * P.n;
+    const uint8_t *sb = L.state + sbase;
+    const uint32_t sid = P.sim_id_base + (uint32_t)b;
+    for (uint32_t w0 = 0; w0 < nblk; w0 += (uint32_t)(CD_WCAP * cs)) {
+        if (tid == 0) sh.nW = 0;
+        __syncthreads();
+        for (uint32_t idx = tid; idx < CD_WCAP; idx += CD_THREADS) {
+            const uint32_t w = w0 + ((idx >> 7) * (uint32_t)cs + (uint32_t)rank) * 128u + (idx & 127u);
+            if (w < nblk && occ_b[w] != 0u) sh.W[atomicAdd(&sh.nW, 1u)] = w;
+        }
+        __syncthreads();
+        const uint32_t nW = sh.nW;
+        for (uint32_t g0 = 0; g0 < nW; g0 += CD_GROUP) {
+            if (tid == 0) sh.nQ = 0;
+            __syncthreads();
+            for (uint32_t pr = tid; pr < CD_GROUP * 32u; pr += CD_THREADS) {          // one (map word, bit) pair per thread
+                const uint32_t wi = g0 + (pr >> 5), bit = pr & 31u;
+                if (wi >= nW) continue;
+                const uint32_t w = sh.W[wi];
+                if (!((occ_b[w] >> bit) & 1u)) continue;
+                const uint32_t site0 = w * 256u + bit * 8u;
+                const unsigned long long v = __ldcg(reinterpret_cast<const unsigned long long *>(sb + site0));
+                uint32_t m = 0;
+#pragma unroll
+                for (int r = 0; r < 8; ++r) {
+                    const uint32_t st = (uint32_t)(v >> (8 * r)) & 0xFFu;
+                    const uint32_t kind = st & 7u;
+                    const bool hit = MODE == 0 ? (kind != CA_EMPTY && kind != CA_WALL) : is_parent(st);
+                    m |= hit ? (1u << r) : 0u;
+                }
+                if (!m) continue;
+                uint32_t pos = atomicAdd(&sh.nQ, (uint32_t)__popc(m));
+                while (m) {
+                    const int r = __ffs(m) - 1;
+                    m &= m - 1;
+                    sh.Q[pos] = site0 + (uint32_t)r;
+                    sh.Qst[pos] = (uint8_t)(v >> (8 * r));
+                    ++pos;
+                }
+            }
+            __syncthreads();
+            const uint32_t nQ = sh.nQ;
+            for (uint32_t r = tid; r < nQ; r += CD_THREADS) {
+                const uint32_t site = sh.Q[r];
+                if (MODE == 0) {
+                    cells_site(P, L, cur, sbase + site, sh.Qst[r], step);
+                } else {
+                    const int dir = detect_decide(P, sb, site, step, sid);
+                    if (dir >= 0) {
+                        const uint32_t slot = atomicAdd(&sh.nwin, 1u);                  // order is irrelevant to the result
+                        if (slot < CD_WINCAP) sh.win[slot] = (site << 3) | (uint32_t)dir;
+                        else *err = CA_EOVERFLOW;
+                    }
+                }
+            }
+            __syncthreads();
+        }
+    }
+}
+
+// grid = batch * cs CTAs in clusters of cs; phases: bit 0 S2, bit 1 S3 (detect + apply)
+__global__ void __launch_bounds__(CD_THREADS) k_cells_divide(KParams P, Lattice L, int cur, const long long *__restrict__ d_step, int k,
+                                                             const uint32_t *__restrict__ occ, int cs, int phases, int *__restrict__ err)
+{
+    __shared__ CDShared sh;
+    const int b = blockIdx.x / cs, rank = blockIdx.x % cs;
+    const uint32_t step = (uint32_t)(*d_step + k);
+    const uint32_t nblk = (uint32_t)(P.n >> 8);
+    const uint32_t *occ_b = occ + (size_t)b * nblk;
+    if (threadIdx.x == 0) sh.nwin = 0;
+    if (phases & 1) cd_pass<0>(P, L, cur, b, rank, cs, step, occ_b, nblk, sh, err);
+    if (phases & 2) {
+        if (cs > 1) cluster_sync_all(); else __syncthreads();                 // every S2 write of this simulation is visible
+        cd_pass<1>(P, L, cur, b, rank, cs, step, occ_b, nblk, sh, err);
+        if (cs > 1) cluster_sync_all(); else __syncthreads();                 // every decision is taken: now write
+        const uint32_t nw = min(sh.nwin, (uint32_t)CD_WINCAP);
+        for (uint32_t w = threadIdx.x; w < nw; w += CD_THREADS) apply_winner(P, L, b, sh.win[w] >> 3, (int)(sh.win[w] & 7u), step);
     }
 }
 
