@@ -42,6 +42,23 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
+def ncu_traffic_bytes():
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of k_diffuse_fused, from the committed ncu summary."""
+    import glob
+    import re
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_ncu_fused_*.txt")))
+    if not files:
+        return None
+    txt = open(files[-1]).read()
+    tot = 0.0
+    for key in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+        m = re.search(key + r"\s+([0-9.]+)\s+(\w+)", txt)
+        if not m:
+            return None
+        tot += float(m.group(1)) * {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}.get(m.group(2), 0.0)
+    return tot
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md clocks line)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -231,9 +248,10 @@ def run_ours(args):
     peak, peak_src = measured_peaks()
     # algorithmic bytes per launch = 25 B x sites x (CA steps one launch completes)
     achieved = B_ALG * B * sites * (1.0 / per_stage_launches) / (launch_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "diffusion-reaction stage S1 (%d launch(es) per CA step)" % round(per_stage_launches),
+    roofline = {"bound": "hbm", "kernel": "k_diffuse_fused: diffusion-reaction stage S1, all n_sub sub-steps (%d launch(es) per CA step)" % round(per_stage_launches),
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
-                "launch_ms": launch_ms, "traffic": None, "stage_share_of_step": stage_ms * S / ms_per_step}
+                "launch_ms": launch_ms, "traffic": ncu_traffic_bytes(), "traffic_unit": "bytes/launch (ncu --set full, profiles/)",
+                "algorithmic_bytes_per_launch": B_ALG * B * sites / per_stage_launches, "stage_share_of_step": stage_ms * S / ms_per_step}
 
     # ---- end to end through the C ABI with HOST buffers: snapshot + protocols up, fitness down, every step
     fit_host = None

@@ -156,7 +156,7 @@ __device__ __forceinline__ void cell_update(const KParams &P, uint32_t &st, uint
 }
 
 // S2 for one occupied site
-__device__ __forceinline__ void cells_site(const KParams &P, const Lattice &L, int cur, long long gi, uint32_t st, uint32_t step)
+__device__ __forceinline__ uint32_t cells_site(const KParams &P, const Lattice &L, int cur, long long gi, uint32_t st, uint32_t step)
 {
     const int b = (int)(gi / P.n);
     const uint32_t i = (uint32_t)(gi - (long long)b * P.n);
@@ -166,6 +166,7 @@ __device__ __forceinline__ void cells_site(const KParams &P, const Lattice &L, i
     if (st != st0) L.state[gi] = (uint8_t)st;
     if (ck != ck0) L.clock[gi] = (uint16_t)ck;
     if (dm != dm0) L.damage[gi] = (uint16_t)dm;
+    return st;
 }
 
 // Sparse scan of the state array shared by S2 and S3.  A persistent grid walks the flat array in 16-byte
@@ -376,17 +377,19 @@ __global__ void __launch_bounds__(256) k_occ_map(const uint8_t *__restrict__ sta
 }
 
 constexpr int CD_THREADS = 512;
-constexpr int CD_WCAP = 4096;     // map words examined per round
+constexpr int CD_WCAP = 2048;     // map words examined per round
+constexpr int CD_TILE = 16;       // map words per interleave tile (one 64x64 plane): CTA rank takes tiles rank, rank + cs, ...
 constexpr int CD_GROUP = 16;      // non-empty map words expanded at a time: at most 16 * 256 = 4096 sites
 constexpr int CD_QCAP = CD_GROUP * 256;
 constexpr int CD_WINCAP = 1024;   // winners per CTA and step
+constexpr int CD_PCAP = 2048;     // READY parents remembered from S2 (more: S3 rescans the map)
 
 struct CDShared {
     uint32_t W[CD_WCAP];          // indices of the non-empty map words of this round
-    uint32_t Q[CD_QCAP];          // sites to work on (index inside the simulation)
-    uint8_t Qst[CD_QCAP];         // their state bytes
+    uint32_t Q[CD_QCAP];          // sites to work on: index into W (11 bits) | byte inside the 256-byte block << 11 | state byte << 19
     uint32_t win[CD_WINCAP];      // winners: parent site << 3 | direction
-    uint32_t nW, nQ, nwin;
+    uint32_t Pl[CD_PCAP];         // READY parents after S2 (site index inside the simulation)
+    uint32_t nW, nQ, nwin, nP;
 };
 
 __device__ __forceinline__ void cluster_sync_all()
@@ -394,8 +397,16 @@ __device__ __forceinline__ void cluster_sync_all()
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
 
-// MODE 0: S2 on every cell of simulation b;  MODE 1: S3 detect on every READY parent.
-// CTA `rank` of `cs` takes the 128-word tiles rank, rank + cs, ... of the simulation's map.
+__device__ __forceinline__ void cd_detect(const KParams &P, const uint8_t *sb, uint32_t site, uint32_t step, uint32_t sid, CDShared &sh, int *err)
+{
+    const int dir = detect_decide(P, sb, site, step, sid);
+    if (dir < 0) return;
+    const uint32_t slot = atomicAdd(&sh.nwin, 1u);                                  // order is irrelevant to the result
+    if (slot < CD_WINCAP) sh.win[slot] = (site << 3) | (uint32_t)dir;
+    else *err = CA_EOVERFLOW;
+}
+
+// MODE 0: S2 on every cell of simulation b (and remember the READY parents);  MODE 1: S3 detect by rescanning the map.
 template <int MODE>
 __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int cur, int b, int rank, int cs, uint32_t step,
                                         const uint32_t *__restrict__ occ_b, uint32_t nblk, CDShared &sh, int *__restrict__ err)
@@ -408,7 +419,7 @@ __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int 
         if (tid == 0) sh.nW = 0;
         __syncthreads();
         for (uint32_t idx = tid; idx < CD_WCAP; idx += CD_THREADS) {
-            const uint32_t w = w0 + ((idx >> 7) * (uint32_t)cs + (uint32_t)rank) * 128u + (idx & 127u);
+            const uint32_t w = w0 + ((idx / CD_TILE) * (uint32_t)cs + (uint32_t)rank) * CD_TILE + (idx % CD_TILE);
             if (w < nblk && occ_b[w] != 0u) sh.W[atomicAdd(&sh.nW, 1u)] = w;
         }
         __syncthreads();
@@ -421,8 +432,7 @@ __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int 
                 if (wi >= nW) continue;
                 const uint32_t w = sh.W[wi];
                 if (!((occ_b[w] >> bit) & 1u)) continue;
-                const uint32_t site0 = w * 256u + bit * 8u;
-                const unsigned long long v = __ldcg(reinterpret_cast<const unsigned long long *>(sb + site0));
+                const unsigned long long v = __ldcg(reinterpret_cast<const unsigned long long *>(sb + (w * 256u + bit * 8u)));
                 uint32_t m = 0;
 #pragma unroll
                 for (int r = 0; r < 8; ++r) {
@@ -436,24 +446,22 @@ __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int 
                 while (m) {
                     const int r = __ffs(m) - 1;
                     m &= m - 1;
-                    sh.Q[pos] = site0 + (uint32_t)r;
-                    sh.Qst[pos] = (uint8_t)(v >> (8 * r));
-                    ++pos;
+                    sh.Q[pos++] = wi | ((bit * 8u + (uint32_t)r) << 11) | (((uint32_t)(v >> (8 * r)) & 0xFFu) << 19);
                 }
             }
             __syncthreads();
             const uint32_t nQ = sh.nQ;
             for (uint32_t r = tid; r < nQ; r += CD_THREADS) {
-                const uint32_t site = sh.Q[r];
+                const uint32_t e = sh.Q[r];
+                const uint32_t site = sh.W[e & 2047u] * 256u + ((e >> 11) & 255u);
                 if (MODE == 0) {
-                    cells_site(P, L, cur, sbase + site, sh.Qst[r], step);
-                } else {
-                    const int dir = detect_decide(P, sb, site, step, sid);
-                    if (dir >= 0) {
-                        const uint32_t slot = atomicAdd(&sh.nwin, 1u);                  // order is irrelevant to the result
-                        if (slot < CD_WINCAP) sh.win[slot] = (site << 3) | (uint32_t)dir;
-                        else *err = CA_EOVERFLOW;
+                    const uint32_t st = cells_site(P, L, cur, sbase + site, e >> 19, step);
+                    if (is_parent(st)) {
+                        const uint32_t slot = atomicAdd(&sh.nP, 1u);
+                        if (slot < CD_PCAP) sh.Pl[slot] = site;
                     }
+                } else {
+                    cd_detect(P, sb, site, step, sid, sh, err);
                 }
             }
             __syncthreads();
@@ -470,11 +478,17 @@ __global__ void __launch_bounds__(CD_THREADS) k_cells_divide(KParams P, Lattice 
     const uint32_t step = (uint32_t)(*d_step + k);
     const uint32_t nblk = (uint32_t)(P.n >> 8);
     const uint32_t *occ_b = occ + (size_t)b * nblk;
-    if (threadIdx.x == 0) sh.nwin = 0;
+    if (threadIdx.x == 0) { sh.nwin = 0; sh.nP = (phases & 1) ? 0u : (uint32_t)CD_PCAP + 1u; }
     if (phases & 1) cd_pass<0>(P, L, cur, b, rank, cs, step, occ_b, nblk, sh, err);
     if (phases & 2) {
         if (cs > 1) cluster_sync_all(); else __syncthreads();                 // every S2 write of this simulation is visible
-        cd_pass<1>(P, L, cur, b, rank, cs, step, occ_b, nblk, sh, err);
+        const uint32_t nP = sh.nP;
+        if (nP <= (uint32_t)CD_PCAP) {                                         // the parents S2 just saw: no second look at the map
+            const uint8_t *sb = L.state + (long long)b * P.n;
+            for (uint32_t r = threadIdx.x; r < nP; r += CD_THREADS) cd_detect(P, sb, sh.Pl[r], step, P.sim_id_base + (uint32_t)b, sh, err);
+        } else {
+            cd_pass<1>(P, L, cur, b, rank, cs, step, occ_b, nblk, sh, err);
+        }
         if (cs > 1) cluster_sync_all(); else __syncthreads();                 // every decision is taken: now write
         const uint32_t nw = min(sh.nwin, (uint32_t)CD_WINCAP);
         for (uint32_t w = threadIdx.x; w < nw; w += CD_THREADS) apply_winner(P, L, b, sh.win[w] >> 3, (int)(sh.win[w] & 7u), step);
