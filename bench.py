@@ -182,6 +182,8 @@ def run_ours(args):
         g.set_option("fused", args.fused)
     if args.graph_steps is not None:
         g.set_option("graph_steps", args.graph_steps)
+    if args.cluster is not None:
+        g.set_option("cluster", args.cluster)
     stream = g.stream
 
     # ---- untimed setup: shared pre-grown spheroid + quasi-steady fields (c2 recipe)
@@ -304,6 +306,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--fused", type=int, default=None)
     ap.add_argument("--graph-steps", type=int, default=None)
+    ap.add_argument("--cluster", type=int, default=None, help="CTAs per simulation of the S2+S3 kernel (1, 2, 4, 8)")
     ap.add_argument("--oracle-steps", type=int, default=600)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

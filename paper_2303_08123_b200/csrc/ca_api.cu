@@ -363,7 +363,7 @@ int ca_create(ca_ctx **out, int batch, int nx, int ny, int nz, const ca_params *
     c->cell_path = 1;
     {
         int cs = 1;
-        while (cs < 8 && (long long)batch * cs * 2 <= 4ll * c->sms && (n >> 8) / CD_TILE >= 8 * cs) cs *= 2;   // up to 4 CTAs per SM, >= 4 planes per CTA
+        while (cs < 8 && (long long)batch * cs * 2 <= 2ll * c->sms && (n >> 8) / CD_TILE >= 8 * cs) cs *= 2;   // about 2 CTAs per SM (measured best at c2: 4 per simulation), >= 4 planes per CTA
         c->cs = cs;
     }
     c->graph[0] = c->graph[1] = nullptr; c->graph_len[0] = c->graph_len[1] = 0; c->graph_nodes = 0; c->launches = 0;
@@ -603,6 +603,10 @@ int ca_set_option(ca_ctx *c, const char *name, int value)
         c->graph_steps = value; drop_graphs(c); return CA_OK;
     }
     if (!std::strcmp(name, "fused")) { c->fused = value ? 1 : 0; drop_graphs(c); return CA_OK; }
+    if (!std::strcmp(name, "cluster")) {
+        if (value != 1 && value != 2 && value != 4 && value != 8) return fail(c, CA_EINVAL, "cluster must be 1, 2, 4 or 8");
+        c->cs = value; drop_graphs(c); return CA_OK;
+    }
     if (!std::strcmp(name, "cell_path")) { c->cell_path = value ? 1 : 0; drop_graphs(c); return CA_OK; }
     return fail(c, CA_EINVAL, std::string("unknown option ") + name);
 }

@@ -168,7 +168,7 @@ struct Fused {
     }
 
     // level K (sub-step K) at iteration i: computes plane t-K; outside the steady range it may idle or copy a WALL plane
-    template <int PH, int K, bool STEADY>
+    template <int PH, int K, bool STEADY, bool NOCELLS>
     static __device__ __forceinline__ void levels(const int t, const uint32_t q, const uint32_t exr, const uint32_t exw,
                                                   u64 (&h)[NL][3][F_PY], FusedCtx &c)
     {
@@ -185,7 +185,7 @@ struct Fused {
                 u64 nloc[F_PY];
                 u64 (&N)[F_PY] = *(K < NL ? &h[KO][sc] : &nloc);
                 level(h[K - 1][sm], h[K - 1][sc], h[K - 1][sp], N, up, dn, c.lam2, c.zero2);
-                if (((c.flags | c.slowmask) >> K) & 1u) {                  // cells in this strip: source term and clamp
+                if (!NOCELLS && (((c.flags | c.slowmask) >> K) & 1u)) {    // cells in this strip: source term and clamp
                     const uint32_t s = c.st_lane + ((q - (uint32_t)K) & (F_SRING - 1)) * (uint32_t)nxny(c);
 #pragma unroll
                     for (int j = 0; j < F_PY; ++j) {
@@ -219,7 +219,7 @@ struct Fused {
                     h[KO][sc][j] = pk(v.x, v.y);
                 }
             }
-            levels<PH, K + 1, STEADY>(t, q, exr, exw, h, c);
+            levels<PH, K + 1, STEADY, NOCELLS>(t, q, exr, exw, h, c);
         }
     }
 
@@ -227,6 +227,15 @@ struct Fused {
     // (slot of plane z = (z - t0) mod 3 on every level)
     template <int PH, bool STEADY>
     static __device__ __forceinline__ void step(const int i, u64 (&h)[NL][3][F_PY], FusedCtx &c)
+    {
+        // most strips of most planes hold no cell: a copy of the steady iteration without any source-term code keeps the
+        // hot loop short (instruction cache) and branch-free
+        if (STEADY && ((c.flags & ((1u << NL) - 1u)) | c.slowmask) == 0u) step_body<PH, true, true>(i, h, c);
+        else step_body<PH, STEADY, false>(i, h, c);
+    }
+
+    template <int PH, bool STEADY, bool NOCELLS>
+    static __device__ __forceinline__ void step_body(const int i, u64 (&h)[NL][3][F_PY], FusedCtx &c)
     {
         const int t = c.t0 + i;
         const uint32_t q = c.itg + (uint32_t)i;
@@ -255,7 +264,7 @@ struct Fused {
                 c.occ_row[(size_t)t * (NX * NY / 256)] = ballot;
         }
         // ---- levels 1..NL: level k computes plane t-k from level k-1
-        levels<PH, 1, STEADY>(t, q, exr, exw, h, c);
+        levels<PH, 1, STEADY, NOCELLS>(t, q, exr, exw, h, c);
         __syncthreads();
     }
 };
