@@ -184,6 +184,10 @@ def run_ours(args):
         g.set_option("graph_steps", args.graph_steps)
     if args.cluster is not None:
         g.set_option("cluster", args.cluster)
+    if args.chains is not None:
+        g.set_option("chains", args.chains)
+    if args.reserve_sms is not None:
+        g.set_option("reserve_sms", args.reserve_sms)
     stream = g.stream
 
     # ---- untimed setup: shared pre-grown spheroid + quasi-steady fields (c2 recipe)
@@ -306,6 +310,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--fused", type=int, default=None)
     ap.add_argument("--graph-steps", type=int, default=None)
+    ap.add_argument("--chains", type=int, default=None)
+    ap.add_argument("--reserve-sms", type=int, default=None)
     ap.add_argument("--cluster", type=int, default=None, help="CTAs per simulation of the S2+S3 kernel (1, 2, 4, 8)")
     ap.add_argument("--oracle-steps", type=int, default=600)
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -82,6 +82,9 @@ struct ca_ctx {
     bool mapped_ok;               // simulations are whole multiples of 256 sites: clustered S2+S3 kernel usable
     int cell_path;                 // option: 1 = clustered S2+S3 kernel when usable, 0 = generic scan kernels
     int cs;                        // CTAs per simulation (cluster size) of the clustered kernel
+    int chains, reserve;           // options: 2 = two concurrent half-batch chains inside a graph; SMs the diffusion kernel leaves free
+    cudaStream_t aux[2];
+    cudaEvent_t ev_fork, ev_join[2];
     // options
     int graph_steps;
     int fused;
@@ -114,6 +117,12 @@ void drop_graphs(ca_ctx *c)
         if (c->graph[q]) { cudaGraphExecDestroy(c->graph[q]); c->graph[q] = nullptr; c->graph_len[q] = 0; }
 }
 
+// two concurrent half-batch chains: only on the fast path (fused fixed-size diffusion + clustered S2+S3)
+bool use_chains(const ca_ctx *c)
+{
+    return c->chains == 2 && c->P.batch >= 2 && c->fused && c->fplan.ok && c->fplan.fixed != 0 && c->mapped_ok && c->cell_path;
+}
+
 inline unsigned int blocks_for(long long n, int threads) { return (unsigned int)((n + threads - 1) / threads); }
 
 // persistent grid of the sparse state scans: 8 CTAs of 8 warps per SM, never more than there are 4 KB trips
@@ -124,37 +133,41 @@ unsigned int scan_grid(const ca_ctx *c)
 }
 
 // S2 and/or S3 through the occupancy map: one cluster of c->cs CTAs per simulation
-void enqueue_cells_divide(ca_ctx *c, int cur, int k, int phases, bool have_map)
+void enqueue_cells_divide(ca_ctx *c, int cur, int k, int phases, bool have_map, int b0 = 0, int nb = -1, cudaStream_t st = nullptr)
 {
+    if (nb < 0) nb = c->P.batch;
+    if (!st) st = c->stream;
     const KParams &P = c->P;
     const long long tot = P.n * P.batch;
     if (!have_map) {
-        k_occ_map<<<blocks_for(tot / 8, 256), 256, 0, c->stream>>>(c->L.state, tot, c->d_occ);
+        k_occ_map<<<blocks_for(tot / 8, 256), 256, 0, st>>>(c->L.state, tot, c->d_occ);   // whole batch (cheap; only on the generic paths)
         c->launches += 1;
     }
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned int)(P.batch * c->cs));
+    cfg.gridDim = dim3((unsigned int)(nb * c->cs));
     cfg.blockDim = dim3(CD_THREADS);
-    cfg.stream = c->stream;
+    cfg.stream = st;
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeClusterDimension;
     at[0].val.clusterDim.x = (unsigned int)c->cs; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
-    cudaLaunchKernelEx(&cfg, k_cells_divide, P, c->L, cur, (const long long *)c->d_step, k, (const uint32_t *)c->d_occ, c->cs, phases, c->d_err);
+    cudaLaunchKernelEx(&cfg, k_cells_divide, P, c->L, cur, (const long long *)c->d_step, k, (const uint32_t *)c->d_occ, c->cs, phases, c->d_err, b0);
     c->launches += 1;
 }
 
 // Enqueue the kernels of ONE CA step (without irradiation) at device step *d_step + k, starting from
 // ping-pong buffer `cur`; returns the buffer holding the fields afterwards.   [D G15]
-int enqueue_step(ca_ctx *c, int cur, int k)
+int enqueue_step(ca_ctx *c, int cur, int k, int b0 = 0, int nb = -1, cudaStream_t st = nullptr, int reserve = 0)
 {
     const KParams &P = c->P;
+    if (nb < 0) nb = P.batch;
+    if (!st) st = c->stream;
     const long long tot = P.n * P.batch;
     const bool mapped = c->mapped_ok && c->cell_path;
     bool have_map = false;
     if (c->fused && fused_supported(c->fplan)) {
         cudaError_t fe;
-        const int np = launch_fused(c->fplan, c->L, cur, mapped ? c->d_occ : nullptr, c->stream, &fe);   // S1: all n_sub sub-steps, one pass over HBM (two if n_sub > 4)
+        const int np = launch_fused(c->fplan, c->L, cur, mapped ? c->d_occ : nullptr, st, &fe, b0, nb, reserve);   // S1: all n_sub sub-steps, one pass over HBM (two if n_sub > 4)
         if (np & 1) cur ^= 1;
         c->launches += np;
         have_map = mapped && c->fplan.fixed != 0;
@@ -166,7 +179,7 @@ int enqueue_step(ca_ctx *c, int cur, int k)
         c->launches += P.n_sub;
     }
     if (mapped) {
-        enqueue_cells_divide(c, cur, k, 3, have_map);                       // S2 + S3 in one clustered launch
+        enqueue_cells_divide(c, cur, k, 3, have_map, b0, nb, st);           // S2 + S3 in one clustered launch
         return cur;
     }
     const ScanArgs sa = { c->d_winners, c->d_nwin + k, c->Y.cap, c->d_err };
@@ -205,7 +218,22 @@ int run_plain(ca_ctx *c, long long nsteps)
             const long long before = c->launches;
             CA_CUDA(c, cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
             int cur = par;
-            for (int k = 0; k < G; ++k) cur = enqueue_step(c, cur, k);
+            if (use_chains(c)) {
+                // Two half-batches on two forked streams.  Simulations never interact, so the halves are independent
+                // chains; while one half is in its latency-bound S2+S3 kernel the other half's diffusion kernel fills
+                // the machine (it leaves c->reserve SMs free so that those CTAs find a home at once).
+                const int half = c->P.batch / 2;
+                CA_CUDA(c, cudaEventRecord(c->ev_fork, c->stream));
+                for (int ch = 0; ch < 2; ++ch) {
+                    CA_CUDA(c, cudaStreamWaitEvent(c->aux[ch], c->ev_fork, 0));
+                    cur = par;
+                    for (int k = 0; k < G; ++k) cur = enqueue_step(c, cur, k, ch * half, ch ? c->P.batch - half : half, c->aux[ch], c->reserve);
+                    CA_CUDA(c, cudaEventRecord(c->ev_join[ch], c->aux[ch]));
+                    CA_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_join[ch], 0));
+                }
+            } else {
+                for (int k = 0; k < G; ++k) cur = enqueue_step(c, cur, k);
+            }
             enqueue_advance(c, G);
             cudaError_t e = cudaStreamEndCapture(c->stream, &g);
             if (e != cudaSuccess) return cuda_fail(c, e, "cudaStreamEndCapture");
@@ -360,6 +388,9 @@ int ca_create(ca_ctx **out, int batch, int nx, int ny, int nz, const ca_params *
     c->fire.assign((size_t)batch * max_frac, 0); c->dose.assign((size_t)batch * max_frac, 0.0f); c->nfrac.assign(batch, 0);
     c->graph_steps = 20; c->fused = 1;
     c->mapped_ok = (n % 256 == 0) && n < (1ll << 29);
+    c->chains = 1; c->reserve = 4;   // two chains measured SLOWER at c2 (137-148 vs 132 us/step): kept as an option only
+    for (int q = 0; q < 2; ++q) { cudaStreamCreateWithFlags(&c->aux[q], cudaStreamNonBlocking); cudaEventCreateWithFlags(&c->ev_join[q], cudaEventDisableTiming); }
+    cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming);
     c->cell_path = 1;
     {
         int cs = 1;
@@ -380,6 +411,8 @@ int ca_destroy(ca_ctx *c)
     if (!c) return CA_OK;
     cudaStreamSynchronize(c->stream);
     drop_graphs(c);
+    for (int q = 0; q < 2; ++q) { cudaStreamDestroy(c->aux[q]); cudaEventDestroy(c->ev_join[q]); }
+    cudaEventDestroy(c->ev_fork);
     if (c->own_stream) cudaStreamDestroy(c->stream);
     delete c;
     return CA_OK;
@@ -603,6 +636,14 @@ int ca_set_option(ca_ctx *c, const char *name, int value)
         c->graph_steps = value; drop_graphs(c); return CA_OK;
     }
     if (!std::strcmp(name, "fused")) { c->fused = value ? 1 : 0; drop_graphs(c); return CA_OK; }
+    if (!std::strcmp(name, "chains")) {
+        if (value != 1 && value != 2) return fail(c, CA_EINVAL, "chains must be 1 or 2");
+        c->chains = value; drop_graphs(c); return CA_OK;
+    }
+    if (!std::strcmp(name, "reserve_sms")) {
+        if (value < 0 || value > 64) return fail(c, CA_EINVAL, "reserve_sms must be 0..64");
+        c->reserve = value; drop_graphs(c); return CA_OK;
+    }
     if (!std::strcmp(name, "cluster")) {
         if (value != 1 && value != 2 && value != 4 && value != 8) return fail(c, CA_EINVAL, "cluster must be 1, 2, 4 or 8");
         c->cs = value; drop_graphs(c); return CA_OK;

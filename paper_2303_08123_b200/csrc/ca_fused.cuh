@@ -25,6 +25,8 @@
 // on its own); v = fma(lambda, lap, c); v += r; max(v, 0).  WALL points use lambda = 0, r = 0, which
 // returns c unchanged.
 #pragma once
+#include <cstdlib>
+#include <cstring>
 #include "ca_device.cuh"
 
 namespace ca {
@@ -35,6 +37,7 @@ constexpr int F_PY = 4;        // rows per lane
 constexpr int F_RING = 3;      // field-plane ring depth = register phase count (prefetch distance 2)
 constexpr int F_SRING = 8;     // state-plane ring depth (a plane is used by NL consecutive iterations)
 constexpr int F_MAXNL = 4;
+constexpr int F_MAXGRID = 640; // persistent CTAs at most (the split table travels as a kernel parameter)
 
 struct FusedArgs {
     const float *src[3];       // current field buffers [batch][nz][ny][nx]
@@ -89,6 +92,7 @@ struct FusedGeom {             // host-computed launch geometry, passed by value
     int nwarps, ngroups_alloc; // strips of F_PY rows: groups = nwarps * (32 / LRP)
     uint32_t off_lut, off_in, off_st, off_ex, smem_bytes;
     long long total_planes;    // batch * 3 * (nz - 2): the flattened (unit, interior plane) space
+    int start[F_MAXGRID + 1];  // CTA g works on flattened planes [start[g], start[g+1]) (cost-balanced on the host)
 };
 
 // per-thread view of one segment (unit = simulation x species, planes [za, zb))
@@ -309,8 +313,8 @@ __global__ void __launch_bounds__(512, 1) k_diffuse_fused(const FusedArgs A, con
     __syncthreads();
 
     const int nzi = A.nz - 2;
-    long long p = Gm.total_planes * (long long)blockIdx.x / gridDim.x;
-    const long long p_end = Gm.total_planes * (long long)(blockIdx.x + 1) / gridDim.x;
+    long long p = Gm.start[blockIdx.x];
+    const long long p_end = Gm.start[blockIdx.x + 1];
     u64 h[NL][3][F_PY];
 #pragma unroll
     for (int k = 0; k < NL; ++k)
@@ -384,12 +388,64 @@ inline size_t fused_smem(int nx, int ny, int nl, int lrp, FusedGeom &G)
     return o;
 }
 
+// Split the flattened (unit, interior plane) space over `grid` CTAs so that every CTA gets the same COST: a segment
+// pays for its planes plus the fill of the NL-level pipeline (cheaper when it starts at a WALL plane, where the
+// empty lead-in iterations are skipped).  Costs in units of one steady iteration, fitted to the measured kernel.
+inline void fused_split(int units, int nzi, int nl, int grid, int *start)
+{
+    static const double f = getenv("CA_RAMP") ? atof(getenv("CA_RAMP")) : 0.55;
+    const double r_wall = f * (2 * nl - 3), r_cut = f * (2 * nl);
+    const long long total = (long long)units * nzi;
+    double lo = 0.0, hi = (double)total + (double)(units + grid) * r_cut + 1.0;
+    for (int it = 0; it < 60; ++it) {                  // smallest per-CTA budget T that covers everything with `grid` CTAs
+        const double T = 0.5 * (lo + hi);
+        long long p = 0;
+        for (int g = 0; g < grid && p < total; ++g) {
+            double used = 0.0;
+            while (p < total) {
+                const int z = (int)(p % nzi);
+                const double r = z == 0 ? r_wall : r_cut;
+                const long long room = (long long)(T - used - r);
+                if (room < 1) break;
+                const long long take = std::min<long long>(room, nzi - z);
+                p += take; used += r + (double)take;
+            }
+        }
+        if (p >= total) hi = T; else lo = T;
+    }
+    long long p = 0;
+    for (int g = 0; g < grid; ++g) {
+        start[g] = (int)p;
+        double used = 0.0;
+        while (p < total) {
+            const int z = (int)(p % nzi);
+            const double r = z == 0 ? r_wall : r_cut;
+            const long long room = (long long)(hi - used - r);
+            if (room < 1) break;
+            const long long take = std::min<long long>(room, nzi - z);
+            p += take; used += r + (double)take;
+        }
+    }
+    start[grid] = (int)total;
+    for (int g = grid - 1; g >= 0 && start[g] > start[grid]; --g) start[g] = start[grid];
+}
+
 template <int NL, int LRP, int NX, int NY>
 inline cudaError_t fused_launch_t(const FusedArgs &A, int grid, cudaStream_t st)
 {
     FusedGeom G{};
     fused_smem(A.nx, A.ny, NL, LRP, G);
     G.total_planes = (long long)A.batch * 3 * (A.nz - 2);
+    if (grid > F_MAXGRID) grid = F_MAXGRID;
+    {   // the split depends on (units, planes, NL, grid) only: keep the last one
+        static int key[4] = { -1, -1, -1, -1 };
+        static int cached[F_MAXGRID + 1];
+        if (key[0] != A.batch || key[1] != A.nz || key[2] != NL || key[3] != grid) {
+            fused_split(A.batch * 3, A.nz - 2, NL, grid, cached);
+            key[0] = A.batch; key[1] = A.nz; key[2] = NL; key[3] = grid;
+        }
+        memcpy(G.start, cached, sizeof(int) * (grid + 1));
+    }
     static bool attr_done = false;      // per instantiation
     if (!attr_done) {
         cudaError_t e = cudaFuncSetAttribute(k_diffuse_fused<NL, LRP, NX, NY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
@@ -441,20 +497,25 @@ inline void fused_configure(const KParams &P, FusedPlan &F)
 inline bool fused_supported(const FusedPlan &F) { return F.ok; }
 
 // Enqueue all n_sub sub-steps starting from ping-pong buffer `cur`; returns the number of passes (= buffer flips).
-inline int launch_fused(FusedPlan &F, const Lattice &L, int cur, uint32_t *occ, cudaStream_t st, cudaError_t *err)
+// Simulations [b0, b0 + nb) only (nb < 0: all); `reserve` SMs are left free for a concurrent chain's S2+S3 kernel.
+inline int launch_fused(FusedPlan &F, const Lattice &L, int cur, uint32_t *occ, cudaStream_t st, cudaError_t *err,
+                        int b0 = 0, int nb = -1, int reserve = 0)
 {
+    if (nb < 0) nb = F.args.batch;
+    const size_t soff = (size_t)b0 * (size_t)F.args.nx * F.args.ny * F.args.nz;
     *err = cudaSuccess;
     for (int ps = 0; ps < F.npass; ++ps) {
         FusedArgs A = F.args;
-        for (int s = 0; s < 3; ++s) { A.src[s] = L.f[cur][s]; A.dst[s] = L.f[cur ^ 1][s]; }
-        A.state = L.state;
-        A.occ = (F.fixed && ps == F.npass - 1) ? occ : nullptr;          // the state does not change between passes: write the map once
+        A.batch = nb;
+        for (int s = 0; s < 3; ++s) { A.src[s] = L.f[cur][s] + soff; A.dst[s] = L.f[cur ^ 1][s] + soff; }
+        A.state = L.state + soff;
+        A.occ = (F.fixed && ps == F.npass - 1 && occ) ? occ + soff / 256 : nullptr;          // the state does not change between passes: write the map once
         FusedGeom G{};
         // CTAs per SM: the 512-thread (nx > 32) kernel fills an SM; smaller lattices use several CTAs per SM
         fused_smem(A.nx, A.ny, F.pass_nl[ps], F.lrp, G);
         const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(std::min<size_t>(4, (227 * 1024) / (G.smem_bytes + 1024)), 512 / (G.nwarps * 32)));
         const long long total = (long long)A.batch * 3 * (A.nz - 2);
-        const int grid = (int)std::max<long long>(1, std::min<long long>((long long)F.sms * per_sm, total / 2 + 1));
+        const int grid = (int)std::max<long long>(1, std::min<long long>((long long)std::max(1, F.sms - reserve) * per_sm, total / 2 + 1));
         cudaError_t e;
         switch (F.pass_nl[ps]) {
         case 1: e = fused_launch_nl<1>(F, A, grid, st); break;

@@ -471,10 +471,10 @@ __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int 
 
 // grid = batch * cs CTAs in clusters of cs; phases: bit 0 S2, bit 1 S3 (detect + apply)
 __global__ void __launch_bounds__(CD_THREADS) k_cells_divide(KParams P, Lattice L, int cur, const long long *__restrict__ d_step, int k,
-                                                             const uint32_t *__restrict__ occ, int cs, int phases, int *__restrict__ err)
+                                                             const uint32_t *__restrict__ occ, int cs, int phases, int *__restrict__ err, int b0)
 {
     __shared__ CDShared sh;
-    const int b = blockIdx.x / cs, rank = blockIdx.x % cs;
+    const int b = b0 + blockIdx.x / cs, rank = blockIdx.x % cs;
     const uint32_t step = (uint32_t)(*d_step + k);
     const uint32_t nblk = (uint32_t)(P.n >> 8);
     const uint32_t *occ_b = occ + (size_t)b * nblk;
