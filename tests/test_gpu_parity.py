@@ -214,3 +214,53 @@ def test_state_roundtrip_broadcast_and_errors():
     cnt = g.counts()
     assert (cnt == np.asarray(r.counts())[None, :]).all()
     g.close()
+
+
+@pytest.mark.parametrize("dims,n_sub,opts", [
+    ((32, 32, 12), 4, {}),                                   # fixed 32x32 kernel, map from the diffusion kernel, default cluster
+    ((64, 64, 10), 4, {"cluster": 1}),                       # fixed 64x64 kernel
+    ((64, 64, 10), 4, {"cluster": 2, "graph_steps": 4}),     # clustered S2+S3 across 2 CTAs, inside CUDA graphs
+    ((64, 64, 10), 4, {"chains": 2, "graph_steps": 4}),      # two half-batch chains on forked streams
+    ((64, 64, 10), 4, {"cell_path": 0}),                     # generic scan kernels next to the fused diffusion
+    ((32, 32, 12), 3, {}),                                   # 3 fused levels
+    ((32, 32, 12), 6, {"graph_steps": 4}),                   # 3 + 3 levels, two passes (buffer flips twice per step)
+    ((32, 32, 12), 5, {"graph_steps": 2}),                   # 3 + 2: odd number of flips per step
+    ((48, 32, 9), 2, {}),                                    # run-time-dims fused kernel, map built by k_occ_map
+])
+def test_fast_path_variants_against_the_oracle(dims, n_sub, opts):
+    """Every launch configuration of the fast path gives the oracle's lattice: bit-exact integers and (against the
+    fp32 build) bit-exact fields over a 60-step window with irradiation, divisions, deaths and lysis; batch of 4."""
+    p = w.stress_params(n_sub=n_sub)
+    seed, base, B = 0xABCD0123, 5, 4
+    g = _gpu(B, dims, p, max_frac=2)
+    for k, v in opts.items():
+        g.set_option(k, v)
+    g.seed("ball", radius=3.4, rng_seed=seed, sim_id_base=base)
+    dose = np.array([[3.0, 2.0], [6.0, 0.5], [0.5, 4.0], [1.0, 1.0]])
+    delay = np.array([[0.01, 0.03], [0.0, 0.05], [0.02, 0.02], [0.03, 0.04]])
+    g.set_protocols(dose, delay)
+    refs = []
+    for b in range(B):
+        pair = []
+        for prec in ("f64", "f32"):
+            r = o.OracleSim(*dims, p, precision=prec)
+            r.seed("ball", radius=3.4, rng_seed=seed, sim_id=base + b)
+            r.set_protocol(dose[b], delay[b])
+            pair.append(r)
+        refs.append(pair)
+    for s in (7, 20, 40, 60):                                 # uneven strides: graphs + single steps + irradiation splits
+        g.run(s / p["steps_per_hour"])
+        for b in range(B):
+            r64, r32 = refs[b]
+            r64.run(s / p["steps_per_hour"]); r32.run(s / p["steps_per_hour"])
+            gs = g.get_state(b)
+            assert_ints_equal(gs, r32.get_state(), "f32 sim %d step %d" % (b, s))
+            assert_fields_bitwise(gs, r32.get_state(), "f32 sim %d step %d" % (b, s))
+            if s <= 50:
+                assert_ints_equal(gs, r64.get_state(), "f64 sim %d step %d" % (b, s))
+            assert_fields_close(gs, r64.get_state(), p, 1e-4, "f64 sim %d step %d" % (b, s))
+    cnt = g.counts()
+    for b in range(B):
+        assert cnt[b].tolist() == refs[b][1].counts().tolist()
+    assert cnt[:, 0].sum() > B * 60 and cnt[:, 1].sum() > 0
+    g.close()
