@@ -49,6 +49,10 @@ struct FusedArgs {
     int always_slow[3];        // 1: the clamp cannot be proven idle for this lambda -> always take the full path
     float zero;                // 0.0f, opaque to ptxas (see Fused::level)
     uint32_t *occ;             // occupancy map for S2/S3 (one bit per 8 state bytes), written by the fixed-size kernels; may be NULL
+    // tiled variant (nx or ny > 64): the plane is cut into ntx * nty tiles of at most 64 x 64 sites including a halo of
+    // F_MAXNL sites towards neighbouring tiles; tile t loads [t0, t1) and stores its output window [o0, o1)
+    int ntx, nty;
+    short tx0[4], tx1[4], ox0[4], ox1[4], ty0[4], ty1[4], oy0[4], oy1[4];
 };
 
 // ---- packed f32x2 arithmetic (Blackwell FADD2/FMUL2/FFMA2); .rn, no ftz: identical to two scalar ops ----
@@ -100,6 +104,7 @@ struct FusedCtx {
     const float *src;          // field of this unit, already offset to this lane's (x0, y0)
     float *dst;
     const float *src_plane0;   // unit base (for the bulk copies)
+    const uint8_t *st_src;     // tiled variant: state of this unit at this lane's (x0, y0)
     const uint8_t *st_plane0;
     int nx, nxny, nz;          // run-time geometry (ignored by the fixed-size instantiations)
     uint32_t ex_lvl;
@@ -121,7 +126,7 @@ struct FusedCtx {
 };
 
 // NX = NY = 0: lattice dims at run time (any even nx <= 2*LRP); otherwise compile-time dims, all address math folds
-template <int NL, int LRP, int NX, int NY>
+template <int NL, int LRP, int NX, int NY, bool TILED = false>
 struct Fused {
     static constexpr bool FIXED = NX != 0;
     static constexpr int RW = 32 / LRP;
@@ -133,6 +138,12 @@ struct Fused {
     static __device__ __forceinline__ int nxny(const FusedCtx &c) { return FIXED ? NX * NY : c.nxny; }
     static __device__ __forceinline__ uint32_t exl(const FusedCtx &c) { return FIXED ? EXL : c.ex_lvl; }
     static __device__ __forceinline__ bool row(const FusedCtx &c, int j) { return FULL ? true : ((c.rowmask >> j) & 1u) != 0u; }
+    // tiled variant: the rings hold a tile with a fixed pitch of 64 sites; only the tile's output window is stored
+    static __device__ __forceinline__ bool srow(const FusedCtx &c, int j) { return TILED ? ((c.rowmask >> (16 + j)) & 1u) != 0u : row(c, j); }
+    static __device__ __forceinline__ uint32_t stpitch(const FusedCtx &c) { return TILED ? 64u : (uint32_t)nx(c); }
+    static __device__ __forceinline__ uint32_t stslot(const FusedCtx &c) { return TILED ? 64u * 64u : (uint32_t)nxny(c); }
+    static __device__ __forceinline__ uint32_t inpitch(const FusedCtx &c) { return TILED ? 256u : (uint32_t)nx(c) * 4u; }
+    static __device__ __forceinline__ uint32_t inslot(const FusedCtx &c) { return TILED ? 64u * 256u : (uint32_t)nxny(c) * 4u; }
 
     // the diffusion part of one sub-step of [D S1] for this lane's 2 x 4 points; C = centre plane, M/P = planes z-1/z+1
     static __device__ __forceinline__ void level(const u64 (&M)[F_PY], const u64 (&C)[F_PY], const u64 (&P)[F_PY], u64 (&N)[F_PY],
@@ -154,6 +165,27 @@ struct Fused {
             const u64 lap = sub2(s6, fma2(six2, C[j], zero2));
             N[j] = fma2(lam2[j], lap, C[j]);                                 // the source term and the clamp follow in levels()
         }
+    }
+
+    // tiled variant: every lane copies its own 4 x 8 field bytes (and, even lanes, 4 x 4 state bytes) of iteration i with
+    // cp.async; one commit group per iteration, empty when there is nothing to load, so that the group count stays uniform
+    static __device__ __forceinline__ void tile_copy(const FusedCtx &c, int i, int slot)
+    {
+        const int t = c.t0 + i;
+        if (i < c.nsteps && t >= c.ld_lo && t < c.ld_hi) {
+            const float *g = c.src + (size_t)t * c.nxny;
+            const uint8_t *gs = c.st_src + (size_t)t * c.nxny;
+            const uint32_t d = c.in_lane + (uint32_t)slot * inslot(c);
+            const uint32_t ds = c.st_lane + ((c.itg + (uint32_t)i) & (F_SRING - 1)) * stslot(c);
+#pragma unroll
+            for (int j = 0; j < F_PY; ++j)
+                if (row(c, j)) {
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d + (uint32_t)j * 256u), "l"(g + j * c.nx) : "memory");
+                    if (!(threadIdx.x & 1))
+                        asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(ds + (uint32_t)j * 64u), "l"(gs + j * c.nx) : "memory");
+                }
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
     }
 
     // producer (one thread): start the bulk copies of iteration i into field-ring slot i mod 3
@@ -190,10 +222,10 @@ struct Fused {
                 u64 (&N)[F_PY] = *(K < NL ? &h[KO][sc] : &nloc);
                 level(h[K - 1][sm], h[K - 1][sc], h[K - 1][sp], N, up, dn, c.lam2, c.zero2);
                 if (!NOCELLS && (((c.flags | c.slowmask) >> K) & 1u)) {    // cells in this strip: source term and clamp
-                    const uint32_t s = c.st_lane + ((q - (uint32_t)K) & (F_SRING - 1)) * (uint32_t)nxny(c);
+                    const uint32_t s = c.st_lane + ((q - (uint32_t)K) & (F_SRING - 1)) * stslot(c);
 #pragma unroll
                     for (int j = 0; j < F_PY; ++j) {
-                        const uint32_t w = row(c, j) ? lds16(s + (uint32_t)(j * nx(c))) : 0u;
+                        const uint32_t w = row(c, j) ? lds16(s + (uint32_t)j * stpitch(c)) : 0u;
                         const u64 v = add2(N[j], pk(lds32f(c.lut + (w & 31u) * 4u), lds32f(c.lut + ((w >> 8) & 31u) * 4u)));
                         float a, b;
                         upk(v, a, b);
@@ -207,7 +239,7 @@ struct Fused {
                     float *o = c.dst + (size_t)zc * nxny(c);
 #pragma unroll
                     for (int j = 0; j < F_PY; ++j)
-                        if (row(c, j)) {
+                        if (srow(c, j)) {
                             float a, b;
                             upk(N[j], a, b);
                             *reinterpret_cast<float2 *>(o + j * nx(c)) = make_float2(a, b);
@@ -243,24 +275,40 @@ struct Fused {
     {
         const int t = c.t0 + i;
         const uint32_t q = c.itg + (uint32_t)i;
-        if (threadIdx.x == 0 && i + (F_RING - 1) < c.nsteps) issue(c, i + (F_RING - 1), (PH + F_RING - 1) % 3);
+        if constexpr (!TILED) {
+            if (threadIdx.x == 0 && i + (F_RING - 1) < c.nsteps) issue(c, i + (F_RING - 1), (PH + F_RING - 1) % 3);
+        }
         const uint32_t exb = exl(c) * NL;                                   // bytes of one exchange buffer
         const uint32_t exw = c.ex_self + ((uint32_t)i & 1u) * exb;          // rows written now, read by the next iteration
         const uint32_t exr = c.ex_self + exb - ((uint32_t)i & 1u) * exb;    // rows written by the previous iteration
         // ---- level 0: plane t from the ring
-        mbar_wait(c.bars + 8u * PH, (c.par >> PH) & 1u);
-        c.par ^= 1u << PH;
+        if constexpr (TILED) {
+            asm volatile("cp.async.wait_group 1;" ::: "memory");             // this iteration's copies have landed (the next one's may be in flight)
+            __syncwarp();                                                   // state bytes are copied by the even lane of each lane pair
+        } else {
+            mbar_wait(c.bars + 8u * PH, (c.par >> PH) & 1u);
+            c.par ^= 1u << PH;
+        }
         bool any = false;
         if (STEADY || (t >= c.ld_lo && t < c.ld_hi)) {
-            const uint32_t a = c.in_lane + (uint32_t)PH * (uint32_t)nxny(c) * 4u;
+            const uint32_t a = c.in_lane + (uint32_t)PH * inslot(c);
 #pragma unroll
-            for (int j = 0; j < F_PY; ++j) h[0][PH][j] = row(c, j) ? lds64(a + (uint32_t)(j * nx(c)) * 4u) : 0ull;
+            for (int j = 0; j < F_PY; ++j) h[0][PH][j] = row(c, j) ? lds64(a + (uint32_t)j * inpitch(c)) : 0ull;
             sts64(exw, h[0][PH][0]);
             sts64(exw + exl(c) / 2, h[0][PH][F_PY - 1]);
             // "cells in my strip": every lane looks at 8 bytes of the warp's strip of the state plane; a byte counts when kind is 1..6
-            const u64 w = c.strip_ok ? lds64(c.st_strip + (q & (F_SRING - 1)) * (uint32_t)nxny(c)) : 0ull;
-            any = (((w & 0x0707070707070707ull) + 0x0101010101010101ull) & 0x0606060606060606ull) != 0ull;
+            if constexpr (TILED) {                                           // tiles are not contiguous: every lane looks at its own 2 x 4 bytes
+                const uint32_t sa = c.st_lane + (q & (F_SRING - 1)) * stslot(c);
+                uint32_t m = 0;
+#pragma unroll
+                for (int j = 0; j < F_PY; ++j) m |= row(c, j) ? (((lds16(sa + (uint32_t)j * 64u) & 0x0707u) + 0x0101u) & 0x0606u) : 0u;
+                any = m != 0u;
+            } else {
+                const u64 w = c.strip_ok ? lds64(c.st_strip + (q & (F_SRING - 1)) * (uint32_t)nxny(c)) : 0ull;
+                any = (((w & 0x0707070707070707ull) + 0x0101010101010101ull) & 0x0606060606060606ull) != 0ull;
+            }
         }
+        if constexpr (TILED) tile_copy(c, i + (F_RING - 1), (PH + F_RING - 1) % 3);   // ring slot of iteration i-1: read one iteration ago
         const uint32_t ballot = __ballot_sync(0xFFFFFFFFu, any);
         c.flags = (c.flags << 1) | (ballot ? 1u : 0u);
         if constexpr (FIXED) {                                              // the same vote is the S2/S3 occupancy map: strip = 256 contiguous bytes
@@ -366,10 +414,104 @@ __global__ void __launch_bounds__(512, 1) k_diffuse_fused(const FusedArgs A, con
     }
 }
 
+// Tiled variant for planes wider than 64 sites (BASELINE configs[2], [3]: 96^3, 80^3).  Same march, same levels; a
+// work unit is (simulation, species, xy-tile, z-range).  A tile carries a halo of F_MAXNL sites towards its neighbour
+// tiles: its outermost ring is frozen (lambda = 0), the garbage that creates moves inwards one site per sub-step and
+// never reaches the output window.  Tiles are not contiguous in memory, so planes arrive by per-lane cp.async
+// (every lane copies exactly the sites it owns: no barrier needed for the field ring).
+template <int NL>
+__global__ void __launch_bounds__(512, 1) k_diffuse_tiled(const FusedArgs A, const FusedGeom Gm)
+{
+    typedef Fused<NL, 32, 0, 0, true> F;
+    extern __shared__ __align__(128) unsigned char fsm[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int lx = lane, g = warp;
+    const uint32_t base = smem_u32(fsm);
+
+    FusedCtx c;
+    c.nx = A.nx; c.nxny = A.nx * A.ny; c.nz = A.nz;
+    c.bars = base; c.in_ring = base + Gm.off_in; c.st_ring = base + Gm.off_st;
+    c.in_lane = c.in_ring + (uint32_t)(F_PY * g) * 256u + (uint32_t)lx * 8u;
+    c.st_lane = c.st_ring + (uint32_t)(F_PY * g) * 64u + (uint32_t)lx * 2u;
+    c.st_strip = 0; c.strip_ok = false; c.occ_row = nullptr; c.src_plane0 = nullptr; c.st_plane0 = nullptr;
+    c.ex_lvl = 2u * (uint32_t)(Gm.ngroups_alloc + 2) * F::GRP;
+    c.ex_self = base + Gm.off_ex + (uint32_t)(g + 1) * F::GRP + (uint32_t)lx * 8u;
+    c.itg = 0; c.par = 0;
+    c.zero2 = pk(A.zero, A.zero);
+    for (int e = tid; e < 96; e += blockDim.x) reinterpret_cast<float *>(fsm + Gm.off_lut)[e] = A.lut[e / 32][e % 32];
+    for (uint32_t e = tid; e < 2u * NL * c.ex_lvl / 8u; e += blockDim.x) reinterpret_cast<u64 *>(fsm + Gm.off_ex)[e] = 0ull;
+    __syncthreads();
+
+    const int nzi = A.nz - 2, ntiles = A.ntx * A.nty;
+    long long p = Gm.start[blockIdx.x];
+    const long long p_end = Gm.start[blockIdx.x + 1];
+    u64 h[NL][3][F_PY];
+#pragma unroll
+    for (int k = 0; k < NL; ++k)
+#pragma unroll
+        for (int s = 0; s < 3; ++s)
+#pragma unroll
+            for (int j = 0; j < F_PY; ++j) h[k][s][j] = 0ull;
+
+    while (p < p_end) {
+        const int unit = (int)(p / nzi);
+        const int tile = unit % ntiles, us = unit / ntiles;
+        const int b = us / 3, sp = us % 3;
+        const int tix = tile % A.ntx, tiy = tile / A.ntx;
+        c.za = 1 + (int)(p - (long long)unit * nzi);
+        c.zb = (int)min((long long)(A.nz - 1), (long long)c.za + (p_end - p));
+        p += c.zb - c.za;
+        const int x = A.tx0[tix] + 2 * lx, y0 = A.ty0[tiy] + F_PY * g;
+        const size_t ubase = (size_t)b * (size_t)c.nxny * (size_t)A.nz;
+        c.src = A.src[sp] + ubase + (y0 * A.nx + x);
+        c.dst = A.dst[sp] + ubase + (y0 * A.nx + x);
+        c.st_src = A.state + ubase + (y0 * A.nx + x);
+        c.t0 = c.za - NL;
+        c.nsteps = c.zb - c.za + 2 * NL;
+        c.ld_lo = max(0, c.za - NL); c.ld_hi = min(A.nz, c.zb + NL);
+        c.st_lo = 2 * NL; c.st_hi = min(A.nz, c.zb + NL) - c.t0;
+        c.flags = 0; c.slowmask = A.always_slow[sp] ? 0xFFFFFFFFu : 0u;
+        c.lut = base + Gm.off_lut + (uint32_t)sp * 128u;
+        const float lam = A.lam[sp];
+        c.rowmask = 0;
+        const bool xin = x < A.tx1[tix];
+        const bool xout = x >= A.ox0[tix] && x < A.ox1[tix];
+#pragma unroll
+        for (int j = 0; j < F_PY; ++j) {
+            const int y = y0 + j;
+            if (xin && y < A.ty1[tiy]) c.rowmask |= 1u << j;
+            if (xout && y >= A.oy0[tiy] && y < A.oy1[tiy]) c.rowmask |= 1u << (16 + j);
+            const bool rowin = y > A.ty0[tiy] && y < A.ty1[tiy] - 1;          // the tile's outer ring is frozen (WALL, or halo edge)
+            c.lam2[j] = pk(rowin && x > A.tx0[tix] && x < A.tx1[tix] - 1 ? lam : 0.0f, rowin && x + 1 < A.tx1[tix] - 1 ? lam : 0.0f);
+        }
+        const int i0 = ((c.ld_lo - c.t0) / 3) * 3;
+        c.t0 += i0; c.nsteps -= i0; c.st_lo = max(0, c.st_lo - i0); c.st_hi -= i0;   // re-base: iteration 0 is the first useful one
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        __syncthreads();                                                     // previous segment done everywhere: rings and exchange are free
+        F::tile_copy(c, 0, 0);
+        F::tile_copy(c, 1, 1);
+        for (int i = 0; i < c.nsteps; i += 3) {
+            if (i >= c.st_lo && i + 3 <= c.st_hi) {
+                F::template step<0, true>(i, h, c);
+                F::template step<1, true>(i + 1, h, c);
+                F::template step<2, true>(i + 2, h, c);
+            } else {
+                F::template step<0, false>(i, h, c);
+                if (i + 1 < c.nsteps) F::template step<1, false>(i + 1, h, c);
+                if (i + 2 < c.nsteps) F::template step<2, false>(i + 2, h, c);
+            }
+        }
+        c.itg += (uint32_t)c.nsteps;
+    }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+}
+
 // ------------------------------------------------------------------ host side --
 struct FusedPlan {
     bool ok = false;
     int lrp = 0, sms = 0, fixed = 0;   // fixed: 0 run-time dims, 32 / 64: the cubic fast instantiations
+    bool tiled = false;                // planes wider than 64 sites: k_diffuse_tiled
+    int tile_warps = 0;
     FusedArgs args{};
     int npass = 0, pass_nl[2] = { 0, 0 };
 };
@@ -457,8 +599,53 @@ inline cudaError_t fused_launch_t(const FusedArgs &A, int grid, cudaStream_t st)
 }
 
 template <int NL>
+inline cudaError_t fused_launch_tiled(const FusedPlan &F, const FusedArgs &A, int grid, cudaStream_t st)
+{
+    FusedGeom G{};
+    fused_smem(64, 64, NL, 32, G);
+    G.nwarps = F.tile_warps;
+    const int units = A.batch * 3 * A.ntx * A.nty;
+    G.total_planes = (long long)units * (A.nz - 2);
+    if (grid > F_MAXGRID) grid = F_MAXGRID;
+    {
+        static int key[4] = { -1, -1, -1, -1 };
+        static int cached[F_MAXGRID + 1];
+        if (key[0] != units || key[1] != A.nz || key[2] != NL || key[3] != grid) {
+            fused_split(units, A.nz - 2, NL, grid, cached);
+            key[0] = units; key[1] = A.nz; key[2] = NL; key[3] = grid;
+        }
+        memcpy(G.start, cached, sizeof(int) * (grid + 1));
+    }
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(k_diffuse_tiled<NL>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    k_diffuse_tiled<NL><<<grid, G.nwarps * 32, G.smem_bytes, st>>>(A, G);
+    return cudaGetLastError();
+}
+
+// cut one lattice dimension into tiles of at most 64 sites including a halo of F_MAXNL towards neighbours; align: cuts on multiples of 4
+inline int fused_tiles(int n, short *t0, short *t1, short *o0, short *o1)
+{
+    for (int nt = 1; nt <= 4; ++nt) {
+        bool ok = true;
+        for (int t = 0; t < nt && ok; ++t) {
+            const int c0 = t == 0 ? 0 : (n * t / nt) / 4 * 4, c1 = t == nt - 1 ? n : (n * (t + 1) / nt) / 4 * 4;
+            t0[t] = (short)std::max(0, c0 - F_MAXNL); t1[t] = (short)std::min(n, c1 + F_MAXNL);
+            o0[t] = (short)c0; o1[t] = (short)c1;
+            ok = t1[t] - t0[t] <= 64 && c1 > c0;
+        }
+        if (ok) return nt;
+    }
+    return 0;
+}
+
+template <int NL>
 inline cudaError_t fused_launch_nl(const FusedPlan &F, const FusedArgs &A, int grid, cudaStream_t st)
 {
+    if (F.tiled) return fused_launch_tiled<NL>(F, A, grid, st);
     if (F.fixed == 64) return fused_launch_t<NL, 32, 64, 64>(A, grid, st);
     if (F.fixed == 32) return fused_launch_t<NL, 16, 32, 32>(A, grid, st);
     if (F.lrp == 16) return fused_launch_t<NL, 16, 0, 0>(A, grid, st);
@@ -469,11 +656,21 @@ inline cudaError_t fused_launch_nl(const FusedPlan &F, const FusedArgs &A, int g
 inline void fused_configure(const KParams &P, FusedPlan &F)
 {
     F.ok = false;
-    if (P.nx % 2 || P.nx > 64 || P.nx < 4 || P.nz < 3 || (P.nx * P.ny) % 16 || P.n_sub < 1 || P.n_sub > 2 * F_MAXNL) return;
+    F.tiled = (P.nx > 64 || P.ny > 64);
+    if (P.nz < 3 || P.n_sub < 1 || P.n_sub > 2 * F_MAXNL || P.nx < 4) return;
+    if (F.tiled) {
+        if (P.nx % 4) return;                                    // 4-byte state copies and 8-byte field copies must stay aligned
+        F.args.ntx = fused_tiles(P.nx, F.args.tx0, F.args.tx1, F.args.ox0, F.args.ox1);
+        F.args.nty = fused_tiles(P.ny, F.args.ty0, F.args.ty1, F.args.oy0, F.args.oy1);
+        if (!F.args.ntx || !F.args.nty) return;
+        int maxh = 0;
+        for (int t = 0; t < F.args.nty; ++t) maxh = std::max(maxh, F.args.ty1[t] - F.args.ty0[t]);
+        F.tile_warps = (maxh + F_PY - 1) / F_PY;
+    } else if (P.nx % 2 || (P.nx * P.ny) % 16) return;
     F.lrp = P.nx <= 32 ? 16 : 32;
     F.fixed = (P.nx == 64 && P.ny == 64) ? 64 : (P.nx == 32 && P.ny == 32) ? 32 : 0;
     FusedGeom G{};
-    if (fused_smem(P.nx, P.ny, F_MAXNL, F.lrp, G) > 227 * 1024 || G.nwarps > 16) return;
+    if (!F.tiled && (fused_smem(P.nx, P.ny, F_MAXNL, F.lrp, G) > 227 * 1024 || G.nwarps > 16)) return;
     int dev = 0;
     cudaDeviceProp prop;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return;
