@@ -130,7 +130,9 @@ template <int NL, int LRP, int NX, int NY, bool TILED = false>
 struct Fused {
     static constexpr bool FIXED = NX != 0;
     static constexpr int RW = 32 / LRP;
-    static constexpr bool FULL = FIXED && NX == 2 * LRP && NY % (F_PY * RW) == 0;    // every lane and row is inside the lattice
+    // every lane and row holds valid data: whole fixed-size planes, or a tile (lanes / strips outside a tile are clamped onto
+    // its last columns / rows: they compute duplicates that feed only the frozen outer ring and are never stored)
+    static constexpr bool FULL = TILED || (FIXED && NX == 2 * LRP && NY % (F_PY * RW) == 0);
     static constexpr uint32_t GRP = LRP * 8u;                                         // bytes of one exchanged row
     static constexpr uint32_t EXL = FIXED ? 2u * (((NY + F_PY * RW - 1) / (F_PY * RW)) * RW + 2u) * GRP : 0u;
 
@@ -462,10 +464,11 @@ __global__ void __launch_bounds__(512, 1) k_diffuse_tiled(const FusedArgs A, con
         c.zb = (int)min((long long)(A.nz - 1), (long long)c.za + (p_end - p));
         p += c.zb - c.za;
         const int x = A.tx0[tix] + 2 * lx, y0 = A.ty0[tiy] + F_PY * g;
+        const int xc = min(x, A.tx1[tix] - 2), yc = min(y0, A.ty1[tiy] - F_PY);   // clamped: always inside the tile
         const size_t ubase = (size_t)b * (size_t)c.nxny * (size_t)A.nz;
-        c.src = A.src[sp] + ubase + (y0 * A.nx + x);
-        c.dst = A.dst[sp] + ubase + (y0 * A.nx + x);
-        c.st_src = A.state + ubase + (y0 * A.nx + x);
+        c.src = A.src[sp] + ubase + (yc * A.nx + xc);
+        c.dst = A.dst[sp] + ubase + (yc * A.nx + xc);                          // stores are masked with the unclamped position
+        c.st_src = A.state + ubase + (yc * A.nx + min(x, A.tx1[tix] - 4));     // even lanes copy 4 state bytes
         c.t0 = c.za - NL;
         c.nsteps = c.zb - c.za + 2 * NL;
         c.ld_lo = max(0, c.za - NL); c.ld_hi = min(A.nz, c.zb + NL);
@@ -659,7 +662,7 @@ inline void fused_configure(const KParams &P, FusedPlan &F)
     F.tiled = (P.nx > 64 || P.ny > 64);
     if (P.nz < 3 || P.n_sub < 1 || P.n_sub > 2 * F_MAXNL || P.nx < 4) return;
     if (F.tiled) {
-        if (P.nx % 4) return;                                    // 4-byte state copies and 8-byte field copies must stay aligned
+        if (P.nx % 4 || P.ny % 4) return;                         // aligned copies; tiles are whole strips of 4 rows                                    // 4-byte state copies and 8-byte field copies must stay aligned
         F.args.ntx = fused_tiles(P.nx, F.args.tx0, F.args.tx1, F.args.ox0, F.args.ox1);
         F.args.nty = fused_tiles(P.ny, F.args.ty0, F.args.ty1, F.args.oy0, F.args.oy1);
         if (!F.args.ntx || !F.args.nty) return;
