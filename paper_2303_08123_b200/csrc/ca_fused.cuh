@@ -134,11 +134,11 @@ struct Fused {
     // its last columns / rows: they compute duplicates that feed only the frozen outer ring and are never stored)
     static constexpr bool FULL = TILED || (FIXED && NX == 2 * LRP && NY % (F_PY * RW) == 0);
     static constexpr uint32_t GRP = LRP * 8u;                                         // bytes of one exchanged row
-    static constexpr uint32_t EXL = FIXED ? 2u * (((NY + F_PY * RW - 1) / (F_PY * RW)) * RW + 2u) * GRP : 0u;
+    static constexpr uint32_t EXL = FIXED ? 2u * (((NY + F_PY * RW - 1) / (F_PY * RW)) * RW + 2u) * GRP : (TILED ? 2u * (16u + 2u) * GRP : 0u);   // tiles: 16 strips allocated
 
     static __device__ __forceinline__ int nx(const FusedCtx &c) { return FIXED ? NX : c.nx; }
     static __device__ __forceinline__ int nxny(const FusedCtx &c) { return FIXED ? NX * NY : c.nxny; }
-    static __device__ __forceinline__ uint32_t exl(const FusedCtx &c) { return FIXED ? EXL : c.ex_lvl; }
+    static __device__ __forceinline__ uint32_t exl(const FusedCtx &c) { return (FIXED || TILED) ? EXL : c.ex_lvl; }
     static __device__ __forceinline__ bool row(const FusedCtx &c, int j) { return FULL ? true : ((c.rowmask >> j) & 1u) != 0u; }
     // tiled variant: the rings hold a tile with a fixed pitch of 64 sites; only the tile's output window is stored
     static __device__ __forceinline__ bool srow(const FusedCtx &c, int j) { return TILED ? ((c.rowmask >> (16 + j)) & 1u) != 0u : row(c, j); }
