@@ -134,7 +134,8 @@ struct Fused {
     // its last columns / rows: they compute duplicates that feed only the frozen outer ring and are never stored)
     static constexpr bool FULL = TILED || (FIXED && NX == 2 * LRP && NY % (F_PY * RW) == 0);
     static constexpr uint32_t GRP = LRP * 8u;                                         // bytes of one exchanged row
-    static constexpr uint32_t EXL = FIXED ? 2u * (((NY + F_PY * RW - 1) / (F_PY * RW)) * RW + 2u) * GRP : (TILED ? 2u * (16u + 2u) * GRP : 0u);   // tiles: 16 strips allocated
+    static constexpr uint32_t EXL = TILED ? 2u * (16u + 2u) * GRP                     // tiles: 16 strips allocated
+                                          : (FIXED ? 2u * (((NY + F_PY * RW - 1) / (F_PY * RW)) * RW + 2u) * GRP : 0u);
 
     static __device__ __forceinline__ int nx(const FusedCtx &c) { return FIXED ? NX : c.nx; }
     static __device__ __forceinline__ int nxny(const FusedCtx &c) { return FIXED ? NX * NY : c.nxny; }
@@ -175,16 +176,16 @@ struct Fused {
     {
         const int t = c.t0 + i;
         if (i < c.nsteps && t >= c.ld_lo && t < c.ld_hi) {
-            const float *g = c.src + (size_t)t * c.nxny;
-            const uint8_t *gs = c.st_src + (size_t)t * c.nxny;
+            const float *g = c.src + (size_t)t * nxny(c);
+            const uint8_t *gs = c.st_src + (size_t)t * nxny(c);
             const uint32_t d = c.in_lane + (uint32_t)slot * inslot(c);
             const uint32_t ds = c.st_lane + ((c.itg + (uint32_t)i) & (F_SRING - 1)) * stslot(c);
 #pragma unroll
             for (int j = 0; j < F_PY; ++j)
                 if (row(c, j)) {
-                    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d + (uint32_t)j * 256u), "l"(g + j * c.nx) : "memory");
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d + (uint32_t)j * 256u), "l"(g + j * nx(c)) : "memory");
                     if (!(threadIdx.x & 1))
-                        asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(ds + (uint32_t)j * 64u), "l"(gs + j * c.nx) : "memory");
+                        asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(ds + (uint32_t)j * 64u), "l"(gs + j * nx(c)) : "memory");
                 }
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
@@ -313,7 +314,7 @@ struct Fused {
         if constexpr (TILED) tile_copy(c, i + (F_RING - 1), (PH + F_RING - 1) % 3);   // ring slot of iteration i-1: read one iteration ago
         const uint32_t ballot = __ballot_sync(0xFFFFFFFFu, any);
         c.flags = (c.flags << 1) | (ballot ? 1u : 0u);
-        if constexpr (FIXED) {                                              // the same vote is the S2/S3 occupancy map: strip = 256 contiguous bytes
+        if constexpr (FIXED && !TILED) {                                    // the same vote is the S2/S3 occupancy map: strip = 256 contiguous bytes
             if ((threadIdx.x & 31) == 0 && c.occ_row != nullptr && (STEADY || (t >= c.ld_lo && t < c.ld_hi)))
                 c.occ_row[(size_t)t * (NX * NY / 256)] = ballot;
         }
@@ -421,10 +422,11 @@ __global__ void __launch_bounds__(512, 1) k_diffuse_fused(const FusedArgs A, con
 // tiles: its outermost ring is frozen (lambda = 0), the garbage that creates moves inwards one site per sub-step and
 // never reaches the output window.  Tiles are not contiguous in memory, so planes arrive by per-lane cp.async
 // (every lane copies exactly the sites it owns: no barrier needed for the field ring).
-template <int NL>
+// NXG, NYG: lattice dims at compile time (row pitch and plane size fold into the copy / store addresses); 0 = run time
+template <int NL, int NXG, int NYG>
 __global__ void __launch_bounds__(512, 1) k_diffuse_tiled(const FusedArgs A, const FusedGeom Gm)
 {
-    typedef Fused<NL, 32, 0, 0, true> F;
+    typedef Fused<NL, 32, NXG, NYG, true> F;
     extern __shared__ __align__(128) unsigned char fsm[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int lx = lane, g = warp;
@@ -601,8 +603,8 @@ inline cudaError_t fused_launch_t(const FusedArgs &A, int grid, cudaStream_t st)
     return cudaGetLastError();
 }
 
-template <int NL>
-inline cudaError_t fused_launch_tiled(const FusedPlan &F, const FusedArgs &A, int grid, cudaStream_t st)
+template <int NL, int NXG, int NYG>
+inline cudaError_t fused_launch_tiled_t(const FusedPlan &F, const FusedArgs &A, int grid, cudaStream_t st)
 {
     FusedGeom G{};
     fused_smem(64, 64, NL, 32, G);
@@ -621,12 +623,20 @@ inline cudaError_t fused_launch_tiled(const FusedPlan &F, const FusedArgs &A, in
     }
     static bool attr_done = false;
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(k_diffuse_tiled<NL>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        cudaError_t e = cudaFuncSetAttribute(k_diffuse_tiled<NL, NXG, NYG>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
-    k_diffuse_tiled<NL><<<grid, G.nwarps * 32, G.smem_bytes, st>>>(A, G);
+    k_diffuse_tiled<NL, NXG, NYG><<<grid, G.nwarps * 32, G.smem_bytes, st>>>(A, G);
     return cudaGetLastError();
+}
+
+template <int NL>
+inline cudaError_t fused_launch_tiled(const FusedPlan &F, const FusedArgs &A, int grid, cudaStream_t st)
+{
+    if (A.nx == 96 && A.ny == 96) return fused_launch_tiled_t<NL, 96, 96>(F, A, grid, st);    // BASELINE configs[2]
+    if (A.nx == 80 && A.ny == 80) return fused_launch_tiled_t<NL, 80, 80>(F, A, grid, st);    // BASELINE configs[3]
+    return fused_launch_tiled_t<NL, 0, 0>(F, A, grid, st);
 }
 
 // cut one lattice dimension into tiles of at most 64 sites including a halo of F_MAXNL towards neighbours; align: cuts on multiples of 4
