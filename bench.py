@@ -28,7 +28,7 @@ if ROOT not in sys.path:
 from paper_2303_08123_b200 import workloads as w   # noqa: E402
 
 B_ALG = 25.0            # algorithmic bytes per site-update (DESIGN.md section 8 / SURVEY 8(d))
-HORIZON_STEPS = 432000  # configs[1]: 30 days at 600 steps/h
+HORIZON_STEPS = 432000  # configs[1], [2]: 30 days at 600 steps/h; configs[3]: 40 days
 
 
 def measured_peaks():
@@ -128,6 +128,24 @@ def oracle_sample(cfg, params, snapshot, steps, sim_id):
     return nx * ny * nz * steps / dt, dt
 
 
+def bench_config(args):
+    """configs[1] (c2) is the headline.  --workload c3s / c4s are REDUCED-BATCH probes of the configs[2] / configs[3]
+    lattices (96^3, 80^3: the tiled diffusion kernel), not headline numbers; config.workload says which one ran."""
+    if args.workload == "c2":
+        return w.config(2)
+    k = 3 if args.workload == "c3s" else 4
+    cfg = dict(w.config(k))
+    batch = 64 if k == 3 else 96
+    cfg["batch"] = batch
+    for key in ("dose", "delay", "nfrac"):
+        cfg[key] = cfg[key][:batch]
+    if k == 3:      # stand-in for the pre-grown 64-site spheroid (DESIGN.md G19): a ball seeded directly, 3 h of warm-up
+        cfg["init"] = dict(kind="ball", center=(48, 48, 48), radius=32.0, shared_init=True)
+        cfg["warmup_h"], cfg["t0_h"] = 3.0, 3.0
+    cfg["name"] += "-reduced"
+    return cfg
+
+
 def run_reference(args):
     """--impl reference: the oracle on the host cores, same metric / unit / config, bounded sample per step."""
     rank = int(os.environ.get("RANK", "0"))
@@ -168,7 +186,7 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
-    cfg = w.config(2)
+    cfg = bench_config(args)
     params = w.default_params()
     B = cfg["batch"]
     nx, ny, nz = cfg["dims"]
@@ -254,9 +272,9 @@ def run_ours(args):
     peak, peak_src = measured_peaks()
     # algorithmic bytes per launch = 25 B x sites x (CA steps one launch completes)
     achieved = B_ALG * B * sites * (1.0 / per_stage_launches) / (launch_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "k_diffuse_fused: diffusion-reaction stage S1, all n_sub sub-steps (%d launch(es) per CA step)" % round(per_stage_launches),
+    roofline = {"bound": "hbm", "kernel": ("k_diffuse_fused" if args.workload == "c2" else "k_diffuse_tiled") + ": diffusion-reaction stage S1, all n_sub sub-steps (%d launch(es) per CA step)" % round(per_stage_launches),
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
-                "launch_ms": launch_ms, "traffic": ncu_traffic_bytes(), "traffic_unit": "bytes/launch (ncu --set full, profiles/)",
+                "launch_ms": launch_ms, "traffic": ncu_traffic_bytes() if args.workload == "c2" else None, "traffic_unit": "bytes/launch (ncu --set full, profiles/)",
                 "algorithmic_bytes_per_launch": B_ALG * B * sites / per_stage_launches, "stage_share_of_step": stage_ms * S / ms_per_step}
 
     # ---- end to end through the C ABI with HOST buffers: snapshot + protocols up, fitness down, every step
@@ -289,10 +307,10 @@ def run_ours(args):
         line = {"metric": "site_updates_per_s", "value": value, "unit": "site-updates/s", "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-                "config": {"workload": "BASELINE configs[1]: %d sims/GPU x %dx%dx%d lattice, shared ~3k-cell spheroid, random 10-fraction protocols" % (B, nx, ny, nz),
-                           "ca_steps_per_step": S, "n_sub": params["n_sub"], "l2": "working set 0.49 GB/GPU > 126 MB L2 (no flush needed)",
+                "config": {"workload": "BASELINE configs[%d]%s: %d sims/GPU x %dx%dx%d lattice, shared spheroid, random protocols" % ({"c2": 1, "c3s": 2, "c4s": 3}[args.workload], "" if args.workload == "c2" else " REDUCED BATCH (probe, not the headline)", B, nx, ny, nz),
+                           "ca_steps_per_step": S, "n_sub": params["n_sub"], "l2": "working set %.2f GB/GPU > 126 MB L2 (no flush needed)" % (29.0 * B * sites / 1e9),
                            "sharding": "batch over ranks, no collective"},
-                "protocols_per_hour": world * B * 3600.0 / (ms_per_step * 1e-3 / S * HORIZON_STEPS),
+                "protocols_per_hour": world * B * 3600.0 / (ms_per_step * 1e-3 / S * (576000 if args.workload == "c4s" else HORIZON_STEPS)),
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
                 "fitness_sample": [float(x) for x in fit_host[:4]]}
         print(json.dumps(line))
@@ -308,6 +326,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--ca-steps", type=int, default=600, help="CA steps per bench step (600 = one simulated hour)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c2", choices=["c2", "c3s", "c4s"], help="c2 = headline; c3s / c4s = reduced-batch probes of the 96^3 / 80^3 lattices")
     ap.add_argument("--fused", type=int, default=None)
     ap.add_argument("--graph-steps", type=int, default=None)
     ap.add_argument("--chains", type=int, default=None)
