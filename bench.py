@@ -146,6 +146,39 @@ def bench_config(args):
     return cfg
 
 
+def run_full_horizon(args):
+    """--full-horizon: evaluate the whole workload to its horizon once (c2: 432 000 CA steps) and report the MEASURED
+    protocols/hour, protocol upload and fitness download included, plus the counts the run ended with."""
+    import torch
+    from paper_2303_08123_b200 import binding
+    cfg = bench_config(args)
+    params = w.default_params()
+    B = cfg["batch"]
+    nx, ny, nz = cfg["dims"]
+    torch.cuda.set_device(0)
+    g = binding.CaBatch(B, nx, ny, nz, params, max_frac=10, device=0)
+    g.seed(rng_seed=cfg["rng_seed"], sim_id_base=0, **cfg["init"])
+    g.run(cfg["warmup_h"])
+    g.sync()
+    t_end = cfg["t0_h"] + cfg["horizon_h"]
+    steps = int(round((t_end - cfg["warmup_h"]) * params["steps_per_hour"]))
+    t0 = time.perf_counter()
+    g.set_protocols(cfg["dose"], cfg["delay"], cfg["nfrac"], t0_h=cfg["t0_h"])
+    g.run(t_end)
+    fit = g.fitness()
+    dt = time.perf_counter() - t0
+    cnt = g.counts()
+    line = {"metric": "protocols_per_hour_measured", "value": B * 3600.0 / dt, "unit": "protocols/h", "n_gpus": 1,
+            "seconds": dt, "ca_steps": steps, "site_updates_per_s": B * nx * ny * nz * steps / dt, "us_per_ca_step": dt / steps * 1e6,
+            "config": {"workload": cfg["name"], "batch": B, "dims": [nx, ny, nz], "horizon_h": cfg["horizon_h"]},
+            "fitness_min_mean_max": [float(fit.min()), float(fit.mean()), float(fit.max())],
+            "live_min_mean_max": [int(cnt[:, 0].min()), float(cnt[:, 0].mean()), int(cnt[:, 0].max())],
+            "occupied_min_mean_max": [int(cnt[:, 12].min()), float(cnt[:, 12].mean()), int(cnt[:, 12].max())],
+            "gpu_launches": g.launch_count, "data": "synthetic"}
+    print(json.dumps(line))
+    g.close()
+
+
 def run_reference(args):
     """--impl reference: the oracle on the host cores, same metric / unit / config, bounded sample per step."""
     rank = int(os.environ.get("RANK", "0"))
@@ -334,10 +367,13 @@ def main():
     ap.add_argument("--cluster", type=int, default=None, help="CTAs per simulation of the S2+S3 kernel (1, 2, 4, 8)")
     ap.add_argument("--oracle-steps", type=int, default=600)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--full-horizon", action="store_true", help="run the whole workload to its horizon once; measured protocols/h")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
-    if args.impl == "reference":
+    if args.full_horizon:
+        run_full_horizon(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

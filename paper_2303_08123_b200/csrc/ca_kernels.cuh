@@ -275,26 +275,42 @@ __global__ void __launch_bounds__(256) k_scan(KParams P, Lattice L, int cur, con
 // lattice and appends the winners (parent, direction) to a list; the apply kernel then writes them.
 //
 // choose_dir: the EMPTY face-neighbour of parent p with the smallest (Philox DIR key, dir); -1 if none.
-__device__ __forceinline__ int choose_dir(const KParams &P, const uint8_t *__restrict__ sb, uint32_t p,
-                                          uint32_t step, uint32_t sid, const int off[6])
+__device__ __forceinline__ uint32_t empty_mask(const uint8_t *__restrict__ sb, uint32_t p, const int off[6])
+{
+    uint32_t nb[6];
+#pragma unroll
+    for (int d = 0; d < 6; ++d) nb[d] = __ldcg(sb + ((int)p + off[d]));   // six independent L2 loads: a neighbour may have been
+    uint32_t em = 0;                                                       // written by another SM in S2
+#pragma unroll
+    for (int d = 0; d < 6; ++d) em |= (nb[d] == CA_EMPTY) ? (1u << d) : 0u;   // WALL != EMPTY: targets are interior
+    return em;
+}
+
+__device__ __forceinline__ int choose_dir_from(const KParams &P, uint32_t em, uint32_t p, uint32_t step, uint32_t sid)
 {
     int best = -1;
     uint32_t bk = 0;
 #pragma unroll
     for (int d = 0; d < 6; ++d) {
-        if (__ldcg(sb + ((int)p + off[d])) != CA_EMPTY) continue;          // WALL != EMPTY: targets are interior.  L2 loads: the
-        const uint32_t kk = rnd(P, p, step, sid, P_DIR, (uint32_t)d);      // neighbour may have been written by another SM in S2
+        if (!((em >> d) & 1u)) continue;
+        const uint32_t kk = rnd(P, p, step, sid, P_DIR, (uint32_t)d);
         if (best < 0 || kk < bk) { best = d; bk = kk; }                    // ties -> lower dir
     }
     return best;
 }
 
+__device__ __forceinline__ int choose_dir(const KParams &P, const uint8_t *__restrict__ sb, uint32_t p,
+                                          uint32_t step, uint32_t sid, const int off[6])
+{
+    return choose_dir_from(P, empty_mask(sb, p, off), p, step, sid);
+}
+
 // Does READY parent p (site index inside its simulation, state array sb) win a target on this step?
 // Returns the direction of its daughter, or -1 (blocked, or lost the claim: untouched, retries next step).
-__device__ __forceinline__ int detect_decide(const KParams &P, const uint8_t *__restrict__ sb, uint32_t p, uint32_t step, uint32_t sid)
+__device__ __forceinline__ int detect_decide_from(const KParams &P, const uint8_t *__restrict__ sb, uint32_t p, uint32_t step, uint32_t sid, uint32_t em)
 {
     const int off[6] = { -1, 1, -P.nx, P.nx, -P.nx * P.ny, P.nx * P.ny };
-    const int dir = choose_dir(P, sb, p, step, sid, off);
+    const int dir = choose_dir_from(P, em, p, step, sid);
     if (dir < 0) return -1;                                                // blocked: stays READY, retries
     const uint32_t e = (uint32_t)((int)p + off[dir]);
     const uint32_t mykey = rnd(P, p, step, sid, P_CLAIM);
@@ -308,6 +324,12 @@ __device__ __forceinline__ int detect_decide(const KParams &P, const uint8_t *__
         if (qk < mykey || (qk == mykey && q < p)) return -1;
     }
     return dir;
+}
+
+__device__ __forceinline__ int detect_decide(const KParams &P, const uint8_t *__restrict__ sb, uint32_t p, uint32_t step, uint32_t sid)
+{
+    const int off[6] = { -1, 1, -P.nx, P.nx, -P.nx * P.ny, P.nx * P.ny };
+    return detect_decide_from(P, sb, p, step, sid, empty_mask(sb, p, off));
 }
 
 __device__ __forceinline__ void detect_site(const KParams &P, const Lattice &L, long long gi, uint32_t step,
@@ -379,17 +401,14 @@ __global__ void __launch_bounds__(256) k_occ_map(const uint8_t *__restrict__ sta
 constexpr int CD_THREADS = 512;
 constexpr int CD_WCAP = 2048;     // map words examined per round
 constexpr int CD_TILE = 16;       // map words per interleave tile (one 64x64 plane): CTA rank takes tiles rank, rank + cs, ...
-constexpr int CD_GROUP = 16;      // non-empty map words expanded at a time: at most 16 * 256 = 4096 sites
-constexpr int CD_QCAP = CD_GROUP * 256;
-constexpr int CD_WINCAP = 1024;   // winners per CTA and step
-constexpr int CD_PCAP = 2048;     // READY parents remembered from S2 (more: S3 rescans the map)
+constexpr int CD_WINCAP = 2048;   // winners per CTA and step
+constexpr int CD_PCAP = 1024;     // READY parents remembered from S2 (more: S3 rescans the map)
 
 struct CDShared {
     uint32_t W[CD_WCAP];          // indices of the non-empty map words of this round
-    uint32_t Q[CD_QCAP];          // sites to work on: index into W (11 bits) | byte inside the 256-byte block << 11 | state byte << 19
     uint32_t win[CD_WINCAP];      // winners: parent site << 3 | direction
     uint32_t Pl[CD_PCAP];         // READY parents after S2 (site index inside the simulation)
-    uint32_t nW, nQ, nwin, nP;
+    uint32_t nW, nwin, nP;
 };
 
 __device__ __forceinline__ void cluster_sync_all()
@@ -397,21 +416,23 @@ __device__ __forceinline__ void cluster_sync_all()
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
 
-__device__ __forceinline__ void cd_detect(const KParams &P, const uint8_t *sb, uint32_t site, uint32_t step, uint32_t sid, CDShared &sh, int *err)
+__device__ __forceinline__ void cd_winner(CDShared &sh, uint32_t site, int dir, int *err)
 {
-    const int dir = detect_decide(P, sb, site, step, sid);
-    if (dir < 0) return;
     const uint32_t slot = atomicAdd(&sh.nwin, 1u);                                  // order is irrelevant to the result
     if (slot < CD_WINCAP) sh.win[slot] = (site << 3) | (uint32_t)dir;
     else *err = CA_EOVERFLOW;
 }
 
-// MODE 0: S2 on every cell of simulation b (and remember the READY parents);  MODE 1: S3 detect by rescanning the map.
+// MODE 0: S2 on every cell of simulation b (READY parents are remembered);  MODE 1: S3 detect by rescanning the map.
+// CTA `rank` of `cs` takes the 16-word tiles rank, rank + cs, ... of the simulation's map.  The CTA compacts the non-empty
+// map words; then every WARP takes half words: 128 consecutive sites = 4 trips of 32 coalesced sites, trips whose 4 map
+// bits are clear are skipped.  All loads of the 4 trips are issued before any site is worked on, so a dense tumour costs
+// about two memory round trips per 128 sites and warp; READY parents first look at their six neighbours (most are blocked).
 template <int MODE>
 __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int cur, int b, int rank, int cs, uint32_t step,
                                         const uint32_t *__restrict__ occ_b, uint32_t nblk, CDShared &sh, int *__restrict__ err)
 {
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const long long sbase = (long long)b * P.n;
     const uint8_t *sb = L.state + sbase;
     const uint32_t sid = P.sim_id_base + (uint32_t)b;
@@ -424,54 +445,64 @@ __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int 
         }
         __syncthreads();
         const uint32_t nW = sh.nW;
-        for (uint32_t g0 = 0; g0 < nW; g0 += CD_GROUP) {
-            if (tid == 0) sh.nQ = 0;
-            __syncthreads();
-            for (uint32_t pr = tid; pr < CD_GROUP * 32u; pr += CD_THREADS) {          // one (map word, bit) pair per thread
-                const uint32_t wi = g0 + (pr >> 5), bit = pr & 31u;
-                if (wi >= nW) continue;
-                const uint32_t w = sh.W[wi];
-                if (!((occ_b[w] >> bit) & 1u)) continue;
-                const unsigned long long v = __ldcg(reinterpret_cast<const unsigned long long *>(sb + (w * 256u + bit * 8u)));
-                uint32_t m = 0;
+        for (uint32_t wi = warp; wi < 2u * nW; wi += CD_THREADS / 32) {      // half a word (4 trips of 32 sites) per warp and turn
+            const uint32_t w = sh.W[wi >> 1];
+            const uint32_t occh = (occ_b[w] >> (16u * (wi & 1u))) & 0xFFFFu;
+            if (!occh) continue;
+            const uint32_t site0 = w * 256u + 128u * (wi & 1u) + (uint32_t)lane;
+            uint32_t st[4];
 #pragma unroll
-                for (int r = 0; r < 8; ++r) {
-                    const uint32_t st = (uint32_t)(v >> (8 * r)) & 0xFFu;
-                    const uint32_t kind = st & 7u;
-                    const bool hit = MODE == 0 ? (kind != CA_EMPTY && kind != CA_WALL) : is_parent(st);
-                    m |= hit ? (1u << r) : 0u;
-                }
-                if (!m) continue;
-                uint32_t pos = atomicAdd(&sh.nQ, (uint32_t)__popc(m));
-                while (m) {
-                    const int r = __ffs(m) - 1;
-                    m &= m - 1;
-                    sh.Q[pos++] = wi | ((bit * 8u + (uint32_t)r) << 11) | (((uint32_t)(v >> (8 * r)) & 0xFFu) << 19);
-                }
-            }
-            __syncthreads();
-            const uint32_t nQ = sh.nQ;
-            for (uint32_t r = tid; r < nQ; r += CD_THREADS) {
-                const uint32_t e = sh.Q[r];
-                const uint32_t site = sh.W[e & 2047u] * 256u + ((e >> 11) & 255u);
-                if (MODE == 0) {
-                    const uint32_t st = cells_site(P, L, cur, sbase + site, e >> 19, step);
-                    if (is_parent(st)) {
-                        const uint32_t slot = atomicAdd(&sh.nP, 1u);
-                        if (slot < CD_PCAP) sh.Pl[slot] = site;
+            for (int r = 0; r < 4; ++r) st[r] = ((occh >> (4 * r)) & 0xFu) ? (uint32_t)__ldcg(sb + site0 + 32u * r) : 0u;
+            if (MODE == 0) {
+                uint32_t ck[4], dm[4];
+                float fo[4], fg[4], fh[4];
+                uint32_t hit = 0;
+#pragma unroll
+                for (int r = 0; r < 4; ++r) {
+                    const uint32_t kind = st[r] & 7u;
+                    if (kind != CA_EMPTY && kind != CA_WALL) {
+                        const long long gi = sbase + site0 + 32u * r;
+                        hit |= 1u << r;
+                        ck[r] = L.clock[gi]; dm[r] = L.damage[gi];
+                        fo[r] = L.f[cur][0][gi]; fg[r] = L.f[cur][1][gi]; fh[r] = L.f[cur][2][gi];
                     }
-                } else {
-                    cd_detect(P, sb, site, step, sid, sh, err);
                 }
+#pragma unroll
+                for (int r = 0; r < 4; ++r)
+                    if ((hit >> r) & 1u) {
+                        const uint32_t i = site0 + 32u * r;
+                        const long long gi = sbase + i;
+                        uint32_t s1 = st[r], c1 = ck[r], d1 = dm[r];
+                        cell_update(P, s1, c1, d1, fo[r], fg[r], fh[r], i, step, sid);
+                        if (s1 != st[r]) L.state[gi] = (uint8_t)s1;
+                        if (c1 != ck[r]) L.clock[gi] = (uint16_t)c1;
+                        if (d1 != dm[r]) L.damage[gi] = (uint16_t)d1;
+                        if (is_parent(s1)) {
+                            const uint32_t slot = atomicAdd(&sh.nP, 1u);
+                            if (slot < CD_PCAP) sh.Pl[slot] = i;
+                        }
+                    }
+            } else {
+                const int off[6] = { -1, 1, -P.nx, P.nx, -P.nx * P.ny, P.nx * P.ny };
+                uint32_t em[4];
+#pragma unroll
+                for (int r = 0; r < 4; ++r) em[r] = is_parent(st[r]) ? empty_mask(sb, site0 + 32u * r, off) : 0u;   // most READY parents are blocked
+#pragma unroll
+                for (int r = 0; r < 4; ++r)
+                    if (em[r]) {
+                        const uint32_t site = site0 + 32u * r;
+                        const int dir = detect_decide_from(P, sb, site, step, sid, em[r]);
+                        if (dir >= 0) cd_winner(sh, site, dir, err);
+                    }
             }
-            __syncthreads();
         }
+        __syncthreads();
     }
 }
 
 // grid = batch * cs CTAs in clusters of cs; phases: bit 0 S2, bit 1 S3 (detect + apply)
-__global__ void __launch_bounds__(CD_THREADS) k_cells_divide(KParams P, Lattice L, int cur, const long long *__restrict__ d_step, int k,
-                                                             const uint32_t *__restrict__ occ, int cs, int phases, int *__restrict__ err, int b0)
+__global__ void __launch_bounds__(CD_THREADS, 2) k_cells_divide(KParams P, Lattice L, int cur, const long long *__restrict__ d_step, int k,
+                                                                const uint32_t *__restrict__ occ, int cs, int phases, int *__restrict__ err, int b0)
 {
     __shared__ CDShared sh;
     const int b = b0 + blockIdx.x / cs, rank = blockIdx.x % cs;
@@ -483,9 +514,12 @@ __global__ void __launch_bounds__(CD_THREADS) k_cells_divide(KParams P, Lattice 
     if (phases & 2) {
         if (cs > 1) cluster_sync_all(); else __syncthreads();                 // every S2 write of this simulation is visible
         const uint32_t nP = sh.nP;
-        if (nP <= (uint32_t)CD_PCAP) {                                         // the parents S2 just saw: no second look at the map
+        if (nP <= (uint32_t)CD_PCAP) {                                         // few parents (small tumour): the ones S2 just saw
             const uint8_t *sb = L.state + (long long)b * P.n;
-            for (uint32_t r = threadIdx.x; r < nP; r += CD_THREADS) cd_detect(P, sb, sh.Pl[r], step, P.sim_id_base + (uint32_t)b, sh, err);
+            for (uint32_t r = threadIdx.x; r < nP; r += CD_THREADS) {
+                const int dir = detect_decide(P, sb, sh.Pl[r], step, P.sim_id_base + (uint32_t)b);
+                if (dir >= 0) cd_winner(sh, sh.Pl[r], dir, err);
+            }
         } else {
             cd_pass<1>(P, L, cur, b, rank, cs, step, occ_b, nblk, sh, err);
         }
