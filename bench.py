@@ -59,6 +59,19 @@ def ncu_traffic_bytes():
     return tot
 
 
+def full_horizon_record():
+    """measured whole-job figure of `bench.py --full-horizon`, as committed under profiles/ (context for the extrapolated one)"""
+    import glob
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_full_horizon_c2.txt")))
+    if not files:
+        return None
+    try:
+        d = json.loads(open(files[-1]).read().strip().splitlines()[-1])
+        return {"protocols_per_hour": d["value"], "us_per_ca_step": d["us_per_ca_step"], "source": os.path.basename(files[-1])}
+    except Exception:
+        return None
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md clocks line)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -344,6 +357,8 @@ def run_ours(args):
                            "ca_steps_per_step": S, "n_sub": params["n_sub"], "l2": "working set %.2f GB/GPU > 126 MB L2 (no flush needed)" % (29.0 * B * sites / 1e9),
                            "sharding": "batch over ranks, no collective"},
                 "protocols_per_hour": world * B * 3600.0 / (ms_per_step * 1e-3 / S * (576000 if args.workload == "c4s" else HORIZON_STEPS)),
+                "protocols_per_hour_note": "extrapolated from the timed CA steps at the start of treatment (~3k-cell tumours); the tumours regrow to ~1.6e5 cells by day 30 and the late steps cost more: see full_horizon_measured",
+                "full_horizon_measured": full_horizon_record() if args.workload == "c2" else None,
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
                 "fitness_sample": [float(x) for x in fit_host[:4]]}
         print(json.dumps(line))
