@@ -435,6 +435,10 @@ __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const long long sbase = (long long)b * P.n;
     const uint8_t *sb = L.state + sbase;
+    uint8_t *stb = L.state + sbase;
+    uint16_t *ckb = L.clock + sbase, *dmb = L.damage + sbase;
+    const float *f0 = L.f[cur][0] + sbase, *f1 = L.f[cur][1] + sbase, *f2 = L.f[cur][2] + sbase;
+    const bool need_dm = (step + 1u) % (uint32_t)P.repair_period == 0u;
     const uint32_t sid = P.sim_id_base + (uint32_t)b;
     for (uint32_t w0 = 0; w0 < nblk; w0 += (uint32_t)(CD_WCAP * cs)) {
         if (tid == 0) sh.nW = 0;
@@ -454,32 +458,54 @@ __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int 
 #pragma unroll
             for (int r = 0; r < 4; ++r) st[r] = ((occh >> (4 * r)) & 0xFu) ? (uint32_t)__ldcg(sb + site0 + 32u * r) : 0u;
             if (MODE == 0) {
-                uint32_t ck[4], dm[4];
+                // Branch-light form of [D S2].  Per step almost every cell only refreshes its mode bits and counts its clock down;
+                // starvation, the end of a countdown and repair are rare and go through cell_update, which recomputes the cell
+                // from its original values (so the two forms cannot disagree).
+                uint32_t ck[4];
                 float fo[4], fg[4], fh[4];
                 uint32_t hit = 0;
 #pragma unroll
                 for (int r = 0; r < 4; ++r) {
                     const uint32_t kind = st[r] & 7u;
                     if (kind != CA_EMPTY && kind != CA_WALL) {
-                        const long long gi = sbase + site0 + 32u * r;
+                        const uint32_t i = site0 + 32u * r;
                         hit |= 1u << r;
-                        ck[r] = L.clock[gi]; dm[r] = L.damage[gi];
-                        fo[r] = L.f[cur][0][gi]; fg[r] = L.f[cur][1][gi]; fh[r] = L.f[cur][2][gi];
+                        ck[r] = ckb[i];
+                        fo[r] = f0[i]; fg[r] = f1[i]; fh[r] = f2[i];
                     }
                 }
 #pragma unroll
                 for (int r = 0; r < 4; ++r)
                     if ((hit >> r) & 1u) {
                         const uint32_t i = site0 + 32u * r;
-                        const long long gi = sbase + i;
-                        uint32_t s1 = st[r], c1 = ck[r], d1 = dm[r];
-                        cell_update(P, s1, c1, d1, fo[r], fg[r], fh[r], i, step, sid);
-                        if (s1 != st[r]) L.state[gi] = (uint8_t)s1;
-                        if (c1 != ck[r]) L.clock[gi] = (uint16_t)c1;
-                        if (d1 != dm[r]) L.damage[gi] = (uint16_t)d1;
-                        if (is_parent(s1)) {
-                            const uint32_t slot = atomicAdd(&sh.nP, 1u);
-                            if (slot < CD_PCAP) sh.Pl[slot] = i;
+                        const uint32_t s0 = st[r], kind = s0 & 7u;
+                        const bool dead = kind == CA_DEAD;
+                        const bool starved = !dead && (fg[r] < P.G_Q || fh[r] > P.H_Q);
+                        const bool prolif = (fg[r] >= P.G_P) && (fh[r] <= P.H_P);
+                        const uint32_t mode = 2u * (uint32_t)(!prolif) + (uint32_t)(!(fo[r] >= P.O_A));
+                        const uint32_t s1 = dead ? s0 : ((s0 & ~0x18u) | (mode << 3));
+                        const bool tick = dead || (prolif && !(s0 & CA_READY));
+                        const uint32_t c1 = ck[r] - (uint32_t)tick;
+                        uint32_t dmv = 0;
+                        if (need_dm && !dead) dmv = dmb[i];                   // repair steps only (uniform) [D G11]
+                        if (starved || (tick && c1 == 0u) || dmv > 0u) {      // rare: the general state machine
+                            uint32_t s2 = s0, c2 = ck[r], d2 = need_dm ? dmv : 1u;   // off repair steps damage can only change to 0 (death, lysis)
+                            const uint32_t d0 = d2;
+                            cell_update(P, s2, c2, d2, fo[r], fg[r], fh[r], i, step, sid);
+                            if (s2 != s0) stb[i] = (uint8_t)s2;
+                            if (c2 != ck[r]) ckb[i] = (uint16_t)c2;
+                            if (d2 != d0) dmb[i] = (uint16_t)d2;
+                            if (is_parent(s2)) {
+                                const uint32_t slot = atomicAdd(&sh.nP, 1u);
+                                if (slot < CD_PCAP) sh.Pl[slot] = i;
+                            }
+                        } else {
+                            if (s1 != s0) stb[i] = (uint8_t)s1;
+                            if (tick) ckb[i] = (uint16_t)c1;
+                            if (is_parent(s1)) {
+                                const uint32_t slot = atomicAdd(&sh.nP, 1u);
+                                if (slot < CD_PCAP) sh.Pl[slot] = i;
+                            }
                         }
                     }
             } else {
