@@ -192,6 +192,38 @@ def run_full_horizon(args):
     g.close()
 
 
+def run_ga_probe(args):
+    """--ga: the configs[4] loop at reduced size -- a population of protocols x 4 seeds streamed through one batch context,
+    host tournament selection + mutation between generations (paper_2303_08123_b200/ga.py).  Reduced horizon and
+    population (stated in the line): a probe of the streaming driver, not the headline."""
+    import torch
+    from paper_2303_08123_b200 import binding, ga
+    cfg = w.config(5)
+    params = w.default_params()
+    nx, ny, nz = cfg["dims"]
+    torch.cuda.set_device(0)
+    B = args.ga_batch
+    g = binding.CaBatch(B, nx, ny, nz, params, max_frac=10, device=0)
+    g.seed(rng_seed=cfg["rng_seed"], sim_id_base=0, **cfg["init"])
+    g.run(cfg["warmup_h"])
+    snap = g.get_state(0)
+    npro, spp = args.ga_population, cfg["seeds_per_protocol"]
+    dose, delay, nfrac = cfg["dose"][:npro], cfg["delay"][:npro], cfg["nfrac"][:npro]
+    t_end = cfg["t0_h"] + args.ga_horizon_h
+    t0 = time.perf_counter()
+    hist, _, fit = ga.run_ga(g, snap, dose, delay, nfrac, args.ga_generations, spp, cfg["rng_seed"], cfg["t0_h"], t_end, ga_seed=cfg["rng_seed"])
+    dt = time.perf_counter() - t0
+    steps = int(round(args.ga_horizon_h * params["steps_per_hour"]))
+    sims = npro * spp * args.ga_generations
+    line = {"metric": "ga_protocol_evaluations_per_hour_reduced_horizon", "value": npro * args.ga_generations * 3600.0 / dt, "unit": "protocols/h",
+            "seconds": dt, "site_updates_per_s": sims * nx * ny * nz * steps / dt,
+            "config": {"workload": "BASELINE configs[4] REDUCED (probe): population %d x %d seeds, %d generations, horizon %.0f h of 720 h, batches of %d on %dx%dx%d"
+                       % (npro, spp, args.ga_generations, args.ga_horizon_h, B, nx, ny, nz)},
+            "best_mean_fitness_per_generation": hist, "data": "synthetic", "gpu_launches": g.launch_count}
+    print(json.dumps(line))
+    g.close()
+
+
 def run_reference(args):
     """--impl reference: the oracle on the host cores, same metric / unit / config, bounded sample per step."""
     rank = int(os.environ.get("RANK", "0"))
@@ -382,11 +414,18 @@ def main():
     ap.add_argument("--cluster", type=int, default=None, help="CTAs per simulation of the S2+S3 kernel (1, 2, 4, 8)")
     ap.add_argument("--oracle-steps", type=int, default=600)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ga", action="store_true", help="configs[4] streaming + host GA loop at reduced size (probe)")
+    ap.add_argument("--ga-population", type=int, default=128)
+    ap.add_argument("--ga-generations", type=int, default=2)
+    ap.add_argument("--ga-horizon-h", type=float, default=12.0)
+    ap.add_argument("--ga-batch", type=int, default=128)
     ap.add_argument("--full-horizon", action="store_true", help="run the whole workload to its horizon once; measured protocols/h")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
-    if args.full_horizon:
+    if args.ga:
+        run_ga_probe(args)
+    elif args.full_horizon:
         run_full_horizon(args)
     elif args.impl == "reference":
         run_reference(args)

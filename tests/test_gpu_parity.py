@@ -267,3 +267,33 @@ def test_fast_path_variants_against_the_oracle(dims, n_sub, opts):
         assert cnt[b].tolist() == refs[b][1].counts().tolist()
     assert cnt[:, 0].sum() > B * 60 and cnt[:, 1].sum() > 0
     g.close()
+
+
+def test_streamed_population_evaluation_is_batch_size_independent():
+    """configs[4] driver: protocols x seeds streamed through a fixed-size batch give, simulation by simulation, the
+    same fitness whatever the batch size, and the same as the oracle started from the same saved tumour."""
+    from paper_2303_08123_b200 import ga
+    p = w.stress_params()
+    dims, seed = (32, 32, 12), 99
+    g0 = _gpu(1, dims, p, max_frac=2)
+    g0.seed("ball", radius=3.0, rng_seed=seed, sim_id_base=0)
+    g0.step(12)
+    snap = g0.get_state(0)
+    g0.close()
+    rng = np.random.default_rng(4)
+    npro, spp = 5, 3
+    dose = rng.choice([0.5, 2.0, 4.0], (npro, 2)); delay = rng.choice([0.01, 0.02, 0.03], (npro, 2)); nfrac = np.full(npro, 2, np.int32)
+    t0 = snap["step"] / p["steps_per_hour"]
+    t_end = t0 + 60 / p["steps_per_hour"]
+    res = []
+    for B in (4, 15, 7):
+        g = _gpu(B, dims, p, max_frac=2)
+        mean, per_sim = ga.evaluate_population(g, snap, dose, delay, nfrac, spp, seed, t0, t_end)
+        res.append(per_sim)
+        g.close()
+    assert np.array_equal(res[0], res[1]) and np.array_equal(res[0], res[2])
+    for sim in (0, 7, 14):                                    # spot-check against the oracle (fp32 build: identical decisions)
+        r = oracle_from_snapshot(snap, p, dims, seed, sim, precision="f32")
+        r.set_protocol(dose[sim // spp], delay[sim // spp], t0_h=t0)
+        r.run(t_end)
+        assert res[0][sim] == r.fitness(), sim
