@@ -275,15 +275,13 @@ __global__ void __launch_bounds__(256) k_scan(KParams P, Lattice L, int cur, con
 // lattice and appends the winners (parent, direction) to a list; the apply kernel then writes them.
 //
 // choose_dir: the EMPTY face-neighbour of parent p with the smallest (Philox DIR key, dir); -1 if none.
-__device__ __forceinline__ uint32_t empty_mask(const uint8_t *__restrict__ sb, uint32_t p, const int off[6])
+__device__ __forceinline__ uint32_t empty_mask(const uint8_t *__restrict__ sb, uint32_t p, int nx, int nxny)
 {
-    uint32_t nb[6];
-#pragma unroll
-    for (int d = 0; d < 6; ++d) nb[d] = __ldcg(sb + ((int)p + off[d]));   // six independent L2 loads: a neighbour may have been
-    uint32_t em = 0;                                                       // written by another SM in S2
-#pragma unroll
-    for (int d = 0; d < 6; ++d) em |= (nb[d] == CA_EMPTY) ? (1u << d) : 0u;   // WALL != EMPTY: targets are interior
-    return em;
+    const uint8_t *q = sb + p;
+    // six independent L2 loads (a neighbour may have been written by another SM in S2); offsets in the order of [D G8]
+    const uint32_t n0 = __ldcg(q - 1), n1 = __ldcg(q + 1), n2 = __ldcg(q - nx), n3 = __ldcg(q + nx), n4 = __ldcg(q - nxny), n5 = __ldcg(q + nxny);
+    return (n0 == CA_EMPTY ? 1u : 0u) | (n1 == CA_EMPTY ? 2u : 0u) | (n2 == CA_EMPTY ? 4u : 0u) | (n3 == CA_EMPTY ? 8u : 0u) |
+           (n4 == CA_EMPTY ? 16u : 0u) | (n5 == CA_EMPTY ? 32u : 0u);          // WALL != EMPTY: targets are interior
 }
 
 __device__ __forceinline__ int choose_dir_from(const KParams &P, uint32_t em, uint32_t p, uint32_t step, uint32_t sid)
@@ -302,7 +300,7 @@ __device__ __forceinline__ int choose_dir_from(const KParams &P, uint32_t em, ui
 __device__ __forceinline__ int choose_dir(const KParams &P, const uint8_t *__restrict__ sb, uint32_t p,
                                           uint32_t step, uint32_t sid, const int off[6])
 {
-    return choose_dir_from(P, empty_mask(sb, p, off), p, step, sid);
+    return choose_dir_from(P, empty_mask(sb, p, P.nx, P.nx * P.ny), p, step, sid);
 }
 
 // Does READY parent p (site index inside its simulation, state array sb) win a target on this step?
@@ -328,8 +326,7 @@ __device__ __forceinline__ int detect_decide_from(const KParams &P, const uint8_
 
 __device__ __forceinline__ int detect_decide(const KParams &P, const uint8_t *__restrict__ sb, uint32_t p, uint32_t step, uint32_t sid)
 {
-    const int off[6] = { -1, 1, -P.nx, P.nx, -P.nx * P.ny, P.nx * P.ny };
-    return detect_decide_from(P, sb, p, step, sid, empty_mask(sb, p, off));
+    return detect_decide_from(P, sb, p, step, sid, empty_mask(sb, p, P.nx, P.nx * P.ny));
 }
 
 __device__ __forceinline__ void detect_site(const KParams &P, const Lattice &L, long long gi, uint32_t step,
@@ -509,10 +506,9 @@ __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int 
                         }
                     }
             } else {
-                const int off[6] = { -1, 1, -P.nx, P.nx, -P.nx * P.ny, P.nx * P.ny };
                 uint32_t em[4];
 #pragma unroll
-                for (int r = 0; r < 4; ++r) em[r] = is_parent(st[r]) ? empty_mask(sb, site0 + 32u * r, off) : 0u;   // most READY parents are blocked
+                for (int r = 0; r < 4; ++r) em[r] = is_parent(st[r]) ? empty_mask(sb, site0 + 32u * r, P.nx, P.nx * P.ny) : 0u;   // most READY parents are blocked
 #pragma unroll
                 for (int r = 0; r < 4; ++r)
                     if (em[r]) {
