@@ -145,9 +145,14 @@ int ca_set_state(ca_ctx *c, int sim_first, int sim_count, const uint8_t *state, 
  * 3 division [D S3].  stage 4 with arg m: m bare diffusion sub-steps. */
 int ca_stage(ca_ctx *c, int stage, int arg);
 
-/* Implementation knobs (not part of the method): name -> value.  "graph_steps" (CA steps per
- * CUDA-graph launch, even, 0 disables graphs), "fused" (1 = temporally fused diffusion kernel,
- * 0 = one launch per sub-step).  CA_EINVAL on an unknown name. */
+/* Implementation knobs (not part of the method; every setting gives bit-identical results): name -> value.
+ *   "graph_steps"  CA steps per CUDA-graph launch (even, 0..64; 0 disables graphs; default 20)
+ *   "fused"        1 = temporally fused diffusion kernels (default), 0 = one launch per sub-step
+ *   "cell_path"    1 = clustered S2+S3 kernel driven by the occupancy map when the lattice allows (default), 0 = generic scans
+ *   "cluster"      CTAs per simulation of the clustered kernel: 1, 2, 4 or 8
+ *   "chains"       2 = two half-batch chains on forked graph branches (measured slower at configs[1]; default 1)
+ *   "reserve_sms"  SMs the diffusion kernel leaves free when chains = 2
+ * CA_EINVAL on an unknown name or value. */
 int ca_set_option(ca_ctx *c, const char *name, int value);
 /* Number of kernel launches (graph nodes included) issued by this context so far. */
 int64_t ca_launch_count(ca_ctx *c);
