@@ -22,7 +22,7 @@ thread_local std::string g_create_error;
 size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 
 struct Layout {
-    size_t field[2][3], state, clock, damage, occ, winners, nwin, step, err, counts, fitness, fire, dose, nfrac, stage, total;
+    size_t field[2][3], state, clock, damage, occ, lys, winners, nwin, step, err, counts, fitness, fire, dose, nfrac, stage, total;
     unsigned int cap;
 };
 
@@ -37,6 +37,7 @@ Layout make_layout(int batch, long long n, int max_frac)
     Y.clock = o;   o = align_up(o + tot * 2);
     Y.damage = o;  o = align_up(o + tot * 2);
     Y.occ = o;     o = align_up(o + (tot / 256 + 64) * 4);   // occupancy map of the S2/S3 fast path
+    Y.lys = o;     o = align_up(o + (size_t)batch * 4);      // per simulation: "a site was vacated (lysis) since S3 last looked"
     size_t cap = std::max<size_t>(65536, tot / 8);
     if (cap > (1u << 28)) cap = 1u << 28;
     Y.cap = (unsigned int)cap;
@@ -79,6 +80,7 @@ struct ca_ctx {
     unsigned long long *d_winners; unsigned int *d_nwin; long long *d_step; int *d_err; int *d_counts; float *d_fitness;
     uint8_t *d_stage;
     uint32_t *d_occ;
+    int *d_lys;
     bool mapped_ok;               // simulations are whole multiples of 256 sites: clustered S2+S3 kernel usable
     int cell_path;                 // option: 1 = clustered S2+S3 kernel when usable, 0 = generic scan kernels
     int cs;                        // CTAs per simulation (cluster size) of the clustered kernel
@@ -151,7 +153,7 @@ void enqueue_cells_divide(ca_ctx *c, int cur, int k, int phases, bool have_map, 
     at[0].id = cudaLaunchAttributeClusterDimension;
     at[0].val.clusterDim.x = (unsigned int)c->cs; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
-    cudaLaunchKernelEx(&cfg, k_cells_divide, P, c->L, cur, (const long long *)c->d_step, k, (const uint32_t *)c->d_occ, c->cs, phases, c->d_err, b0);
+    cudaLaunchKernelEx(&cfg, k_cells_divide, P, c->L, cur, (const long long *)c->d_step, k, (const uint32_t *)c->d_occ, c->cs, phases, c->d_err, b0, c->d_lys);
     c->launches += 1;
 }
 
@@ -374,6 +376,7 @@ int ca_create(ca_ctx **out, int batch, int nx, int ny, int nz, const ca_params *
     c->d_nfrac = (int *)(c->ws + c->Y.nfrac);
     c->d_stage = c->ws + c->Y.stage;
     c->d_occ = (uint32_t *)(c->ws + c->Y.occ);
+    c->d_lys = (int *)(c->ws + c->Y.lys);
     c->stream = (cudaStream_t)stream;
     c->own_stream = false;
     if (!c->stream) {                     // the legacy default stream cannot be captured into CUDA graphs
@@ -400,6 +403,7 @@ int ca_create(ca_ctx **out, int batch, int nx, int ny, int nz, const ca_params *
     c->graph[0] = c->graph[1] = nullptr; c->graph_len[0] = c->graph_len[1] = 0; c->graph_nodes = 0; c->launches = 0;
     // zero the small control blocks (protocol tables, counters)
     e = cudaMemsetAsync(c->ws + c->Y.winners, 0, c->Y.total - c->Y.winners, c->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->d_lys, 1, (size_t)batch * 4, c->stream);
     if (e != cudaSuccess) { int rc = cuda_fail(nullptr, e, "cudaMemsetAsync"); delete c; return rc; }
     fused_configure(P, c->fplan);
     *out = c;
@@ -544,7 +548,10 @@ int ca_get_state(ca_ctx *c, int sim, uint8_t *state, uint16_t *clock, uint16_t *
     for (int s = 0; s < 3; ++s)
         if (dst[s]) CA_CUDA(c, cudaMemcpyAsync(dst[s], c->L.f[c->cur][s] + o, n * 4, cudaMemcpyDeviceToHost, c->stream));
     if (step) *step = (int64_t)c->step;
-    return check_deferred(c);
+    const int rc = check_deferred(c);                                       // synchronises: the copies have landed
+    if (rc == CA_OK && state)
+        for (size_t i = 0; i < n; ++i) state[i] &= 0x7Fu;                   // bit 7 is internal ("known to be blocked", see k_cells_divide)
+    return rc;
 }
 
 int ca_set_state(ca_ctx *c, int sim_first, int sim_count, const uint8_t *state, const uint16_t *clock, const uint16_t *damage,
@@ -648,7 +655,11 @@ int ca_set_option(ca_ctx *c, const char *name, int value)
         if (value != 1 && value != 2 && value != 4 && value != 8) return fail(c, CA_EINVAL, "cluster must be 1, 2, 4 or 8");
         c->cs = value; drop_graphs(c); return CA_OK;
     }
-    if (!std::strcmp(name, "cell_path")) { c->cell_path = value ? 1 : 0; drop_graphs(c); return CA_OK; }
+    if (!std::strcmp(name, "cell_path")) {
+        c->cell_path = value ? 1 : 0; drop_graphs(c);
+        cudaMemsetAsync(c->d_lys, 1, (size_t)c->P.batch * 4, c->stream);     // the generic path does not track lysis: re-evaluate every parent once
+        return CA_OK;
+    }
     return fail(c, CA_EINVAL, std::string("unknown option ") + name);
 }
 

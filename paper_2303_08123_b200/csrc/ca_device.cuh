@@ -75,6 +75,9 @@ __device__ __forceinline__ uint16_t draw_clock(const KParams &P, int kind, uint3
     return (uint16_t)(T - J + (int)uniform_int(rnd(P, site, step, sid, purpose), (uint32_t)(2 * J + 1)));
 }
 
+// internal state bit 7 (never exported): READY parent known to have no EMPTY neighbour  (k_cells_divide)
+constexpr uint32_t CA_BLOCKED = 0x80u;
+
 __device__ __forceinline__ bool is_live(uint32_t st) { const uint32_t k = st & 7u; return k >= 1u && k <= 4u; }
 // READY parent able to divide: kind M, READY, proliferating mode (< 2)  [D S3 step 1]
 __device__ __forceinline__ bool is_parent(uint32_t st) { return (st & 0x37u) == (uint32_t)(CA_M | CA_READY); }

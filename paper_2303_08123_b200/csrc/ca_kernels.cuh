@@ -427,7 +427,8 @@ __device__ __forceinline__ void cd_winner(CDShared &sh, uint32_t site, int dir, 
 // about two memory round trips per 128 sites and warp; READY parents first look at their six neighbours (most are blocked).
 template <int MODE>
 __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int cur, int b, int rank, int cs, uint32_t step,
-                                        const uint32_t *__restrict__ occ_b, uint32_t nblk, CDShared &sh, int *__restrict__ err)
+                                        const uint32_t *__restrict__ occ_b, uint32_t nblk, CDShared &sh, int *__restrict__ err,
+                                        int *__restrict__ lys_b, bool trust)
 {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const long long sbase = (long long)b * P.n;
@@ -489,26 +490,34 @@ __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int 
                             uint32_t s2 = s0, c2 = ck[r], d2 = need_dm ? dmv : 1u;   // off repair steps damage can only change to 0 (death, lysis)
                             const uint32_t d0 = d2;
                             cell_update(P, s2, c2, d2, fo[r], fg[r], fh[r], i, step, sid);
+                            if ((s2 & 7u) == CA_EMPTY) *lys_b = 1;               // a site was vacated: blocked parents must look again
                             if (s2 != s0) stb[i] = (uint8_t)s2;
                             if (c2 != ck[r]) ckb[i] = (uint16_t)c2;
                             if (d2 != d0) dmb[i] = (uint16_t)d2;
                             if (is_parent(s2)) {
                                 const uint32_t slot = atomicAdd(&sh.nP, 1u);
-                                if (slot < CD_PCAP) sh.Pl[slot] = i;
+                                if (slot < CD_PCAP) sh.Pl[slot] = i | ((s2 & CA_BLOCKED) << 24);
                             }
                         } else {
                             if (s1 != s0) stb[i] = (uint8_t)s1;
                             if (tick) ckb[i] = (uint16_t)c1;
                             if (is_parent(s1)) {
                                 const uint32_t slot = atomicAdd(&sh.nP, 1u);
-                                if (slot < CD_PCAP) sh.Pl[slot] = i;
+                                if (slot < CD_PCAP) sh.Pl[slot] = i | ((s1 & CA_BLOCKED) << 24);
                             }
                         }
                     }
             } else {
                 uint32_t em[4];
 #pragma unroll
-                for (int r = 0; r < 4; ++r) em[r] = is_parent(st[r]) ? empty_mask(sb, site0 + 32u * r, P.nx, P.nx * P.ny) : 0u;   // most READY parents are blocked
+                for (int r = 0; r < 4; ++r) {
+                    em[r] = 0u;
+                    if (is_parent(st[r]) && !(trust && (st[r] & CA_BLOCKED))) {        // most READY parents are blocked, and known to be
+                        em[r] = empty_mask(sb, site0 + 32u * r, P.nx, P.nx * P.ny);
+                        const uint32_t nb = em[r] ? (st[r] & ~CA_BLOCKED) : (st[r] | CA_BLOCKED);
+                        if (nb != st[r]) L.state[sbase + site0 + 32u * r] = (uint8_t)nb;
+                    }
+                }
 #pragma unroll
                 for (int r = 0; r < 4; ++r)
                     if (em[r]) {
@@ -524,7 +533,7 @@ __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int 
 
 // grid = batch * cs CTAs in clusters of cs; phases: bit 0 S2, bit 1 S3 (detect + apply)
 __global__ void __launch_bounds__(CD_THREADS, 2) k_cells_divide(KParams P, Lattice L, int cur, const long long *__restrict__ d_step, int k,
-                                                                const uint32_t *__restrict__ occ, int cs, int phases, int *__restrict__ err, int b0)
+                                                                const uint32_t *__restrict__ occ, int cs, int phases, int *__restrict__ err, int b0, int *__restrict__ lys)
 {
     __shared__ CDShared sh;
     const int b = b0 + blockIdx.x / cs, rank = blockIdx.x % cs;
@@ -532,22 +541,33 @@ __global__ void __launch_bounds__(CD_THREADS, 2) k_cells_divide(KParams P, Latti
     const uint32_t nblk = (uint32_t)(P.n >> 8);
     const uint32_t *occ_b = occ + (size_t)b * nblk;
     if (threadIdx.x == 0) { sh.nwin = 0; sh.nP = (phases & 1) ? 0u : (uint32_t)CD_PCAP + 1u; }
-    if (phases & 1) cd_pass<0>(P, L, cur, b, rank, cs, step, occ_b, nblk, sh, err);
+    if (phases & 1) cd_pass<0>(P, L, cur, b, rank, cs, step, occ_b, nblk, sh, err, lys + b, false);
     if (phases & 2) {
         if (cs > 1) cluster_sync_all(); else __syncthreads();                 // every S2 write of this simulation is visible
+        // A READY parent found without an EMPTY neighbour stays blocked until a site of its simulation is vacated, and
+        // that only happens by lysis in S2.  Bit 7 of its state byte remembers "blocked" (internal: masked on export); it
+        // is trusted on steps on which no lysis happened since it was written, and refreshed otherwise.
+        const bool trust = *(volatile int *)(lys + b) == 0;
         const uint32_t nP = sh.nP;
         if (nP <= (uint32_t)CD_PCAP) {                                         // few parents (small tumour): the ones S2 just saw
-            const uint8_t *sb = L.state + (long long)b * P.n;
+            const long long sbase = (long long)b * P.n;
+            const uint8_t *sb = L.state + sbase;
             for (uint32_t r = threadIdx.x; r < nP; r += CD_THREADS) {
-                const int dir = detect_decide(P, sb, sh.Pl[r], step, P.sim_id_base + (uint32_t)b);
-                if (dir >= 0) cd_winner(sh, sh.Pl[r], dir, err);
+                const uint32_t site = sh.Pl[r] & 0x7FFFFFFFu, was = sh.Pl[r] >> 31;
+                if (trust && was) continue;
+                const uint32_t em = empty_mask(sb, site, P.nx, P.nx * P.ny);
+                if ((em == 0u) != (was != 0u)) L.state[sbase + site] = (uint8_t)(em ? (__ldcg(sb + site) & ~CA_BLOCKED) : (__ldcg(sb + site) | CA_BLOCKED));
+                if (!em) continue;
+                const int dir = detect_decide_from(P, sb, site, step, P.sim_id_base + (uint32_t)b, em);
+                if (dir >= 0) cd_winner(sh, site, dir, err);
             }
         } else {
-            cd_pass<1>(P, L, cur, b, rank, cs, step, occ_b, nblk, sh, err);
+            cd_pass<1>(P, L, cur, b, rank, cs, step, occ_b, nblk, sh, err, lys + b, trust);
         }
         if (cs > 1) cluster_sync_all(); else __syncthreads();                 // every decision is taken: now write
         const uint32_t nw = min(sh.nwin, (uint32_t)CD_WINCAP);
         for (uint32_t w = threadIdx.x; w < nw; w += CD_THREADS) apply_winner(P, L, b, sh.win[w] >> 3, (int)(sh.win[w] & 7u), step);
+        if (rank == 0 && threadIdx.x == 0) lys[b] = 0;                        // every CTA of the cluster read it before the second barrier
     }
 }
 
