@@ -481,7 +481,8 @@ __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int 
                         const bool starved = !dead && (fg[r] < P.G_Q || fh[r] > P.H_Q);
                         const bool prolif = (fg[r] >= P.G_P) && (fh[r] <= P.H_P);
                         const uint32_t mode = 2u * (uint32_t)(!prolif) + (uint32_t)(!(fo[r] >= P.O_A));
-                        const uint32_t s1 = dead ? s0 : ((s0 & ~0x18u) | (mode << 3));
+                        uint32_t s1 = dead ? s0 : ((s0 & ~0x18u) | (mode << 3));
+                        if (!is_parent(s1)) s1 &= ~CA_BLOCKED;               // "blocked" is only remembered while the cell stays a parent (see S3)
                         const bool tick = dead || (prolif && !(s0 & CA_READY));
                         const uint32_t c1 = ck[r] - (uint32_t)tick;
                         uint32_t dmv = 0;
@@ -491,6 +492,7 @@ __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int 
                             const uint32_t d0 = d2;
                             cell_update(P, s2, c2, d2, fo[r], fg[r], fh[r], i, step, sid);
                             if ((s2 & 7u) == CA_EMPTY) *lys_b = 1;               // a site was vacated: blocked parents must look again
+                            if (!is_parent(s2)) s2 &= ~CA_BLOCKED;
                             if (s2 != s0) stb[i] = (uint8_t)s2;
                             if (c2 != ck[r]) ckb[i] = (uint16_t)c2;
                             if (d2 != d0) dmb[i] = (uint16_t)d2;

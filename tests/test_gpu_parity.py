@@ -297,3 +297,39 @@ def test_streamed_population_evaluation_is_batch_size_independent():
         r.set_protocol(dose[sim // spp], delay[sim // spp], t0_h=t0)
         r.run(t_end)
         assert res[0][sim] == r.fitness(), sim
+
+
+def test_dense_starving_tumour_long_window_all_cell_paths_agree():
+    """A dense spheroid with strong uptake: quiescent READY cells, starvation deaths, lysis, blocked parents that become
+    unblocked -- the situations the blocked-parent memory of the clustered kernel has to get right.  The oracle (fp32
+    build) is followed for 240 steps, the generic and the clustered GPU paths are compared bit for bit over 900."""
+    p = w.stress_params(lysis_steps=25)
+    p["rate"] = [[-4e-3, 0.0, -2e-3, 0.0], [-2.4e-2, -7e-2, -1.2e-2, -3.5e-2], [1.5e-7, 6e-7, 0.75e-7, 3e-7]]
+    dims, seed, B = (32, 32, 32), 777, 3
+    dose = np.array([[2.0, 3.0]] * B); delay = np.array([[0.25, 0.5]] * B)
+    runs = []
+    for cell_path in (1, 0):
+        g = _gpu(B, dims, p, max_frac=2)
+        g.set_option("cell_path", cell_path)
+        g.seed("ball", radius=8.5, rng_seed=seed, sim_id_base=40)
+        g.set_protocols(dose, delay)
+        snaps = []
+        for s in (240, 600, 900):
+            g.run(s / p["steps_per_hour"])
+            snaps.append([g.get_state(b) for b in range(B)])
+        runs.append((snaps, g.counts()))
+        g.close()
+    (sa, ca_), (sb_, cb) = runs
+    assert np.array_equal(ca_, cb)
+    for k in range(3):
+        for b in range(B):
+            assert_ints_equal(sa[k][b], sb_[k][b], "paths, window %d sim %d" % (k, b))
+            assert_fields_bitwise(sa[k][b], sb_[k][b], "paths, window %d sim %d" % (k, b))
+    c = ca_.sum(0)
+    assert c[3] > 0 and c[2] > 0 and (c[10] + c[11]) > 0, c          # dead cells, READY cells, quiescent cells all present
+    r = o.OracleSim(*dims, p, precision="f32")
+    r.seed("ball", radius=8.5, rng_seed=seed, sim_id=41)
+    r.set_protocol(dose[1], delay[1])
+    r.run(240 / p["steps_per_hour"])
+    assert_ints_equal(sa[0][1], r.get_state(), "oracle f32, 240 steps")
+    assert_fields_bitwise(sa[0][1], r.get_state(), "oracle f32, 240 steps")
