@@ -104,3 +104,34 @@ def test_c2_shape_100_hours_fast_path_equals_generic_path():
     for b in range(B):
         for k in ("state", "clock", "damage", "o2", "glc", "h"):
             assert np.array_equal(sa[b][k], sb[b][k]), (b, k)
+
+
+@pytest.mark.parametrize("k,batch,dims", [(3, 512, (96, 96, 96)), (4, 1024, (80, 80, 80))])
+def test_c3_c4_full_batch_size_window_against_the_oracle(k, batch, dims):
+    """configs[2] / configs[3] at their FULL batch size (13 / 15 GB of lattice state: 64-bit indexing, tiled diffusion
+    kernel, occupancy map, clusters): a 30-step window from ca_seed with one fraction inside, first / middle / last
+    simulation against the fp32 and fp64 oracles."""
+    p = w.default_params()
+    cfg = w.config(k)
+    g = binding.CaBatch(batch, *dims, p, max_frac=8)
+    g.seed("ball", radius=12.0, rng_seed=cfg["rng_seed"], sim_id_base=0, shared_init=False)
+    dose = np.full((batch, 1), 2.0); dose[-1, 0] = 6.0
+    delay = np.full((batch, 1), 10.0 / p["steps_per_hour"])
+    g.set_protocols(dose, delay)
+    g.step(30)
+    cnt = g.counts()
+    assert cnt[:, 0].min() > 6000 and cnt[:, 1].min() > 0
+    for b in (0, batch // 2 + 1, batch - 1):
+        gs = g.get_state(b)
+        for prec in ("f32", "f64"):
+            r = o.OracleSim(*dims, p, precision=prec)
+            r.seed("ball", radius=12.0, rng_seed=cfg["rng_seed"], sim_id=b)
+            r.set_protocol(dose[b], delay[b])
+            r.step(30)
+            assert_ints_equal(gs, r.get_state(), "%s sim %d" % (prec, b))
+            if prec == "f32":
+                assert_fields_bitwise(gs, r.get_state(), "f32 sim %d" % b)
+                assert cnt[b].tolist() == r.counts().tolist()
+            else:
+                assert_fields_close(gs, r.get_state(), p, 1e-4, "f64 sim %d" % b)
+    g.close()
