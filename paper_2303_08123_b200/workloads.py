@@ -133,3 +133,35 @@ def config(k):
                     init=dict(kind="ball", center=(32, 32, 32), radius=9.0, shared_init=True),
                     warmup_h=6.0, t0_h=6.0, horizon_h=720.0, dose=dose, delay=delay, nfrac=nfrac)
     raise ValueError("config index must be 1..5")
+
+
+def robustness_sweep(base_dose, base_delay, shifts_h=(-1.0, -0.5, 0.5, 1.0), step_h=0.5):
+    """NEXT-4 workload (how sensitive is a good protocol to delivery errors?): every variant of one
+    protocol in which a single fraction is dropped, or delivered `shift` hours early / late (the following fraction
+    keeps its absolute time).  Returns (dose, delay, nfrac, labels); row 0 is the unperturbed protocol.  Delays stay on
+    the `step_h` grid and non-negative; variants that would leave it are skipped."""
+    base_dose = np.asarray(base_dose, dtype=np.float64)
+    base_delay = np.asarray(base_delay, dtype=np.float64)
+    k = len(base_dose)
+    rows, labels = [(base_dose.copy(), base_delay.copy(), k)], ["base"]
+    for j in range(k):                                              # drop fraction j: its delay is added to the next one
+        d = np.delete(base_dose, j)
+        t = np.delete(base_delay, j)
+        if j < k - 1:
+            t[j] += base_delay[j]
+        rows.append((np.append(d, 0.0), np.append(t, 0.0), k - 1))
+        labels.append("drop%d" % j)
+    for j in range(k):
+        for s in shifts_h:
+            t = base_delay.copy()
+            t[j] += s
+            if j < k - 1:
+                t[j + 1] -= s
+            if t.min() < 0 or abs(s / step_h - round(s / step_h)) > 1e-9:
+                continue
+            rows.append((base_dose.copy(), t, k))
+            labels.append("shift%d%+.1fh" % (j, s))
+    dose = np.stack([r[0] for r in rows])
+    delay = np.stack([r[1] for r in rows])
+    nfrac = np.array([r[2] for r in rows], np.int32)
+    return dose, delay, nfrac, labels

@@ -33,3 +33,21 @@ def test_selection_prefers_fitter_parents_and_is_reproducible():
     nd, nt, _ = a
     parent = [int(np.argmin((nd[c][None, :] != dose).sum(1) + (nt[c][None, :] != delay).sum(1))) for c in range(20, 200)]
     assert np.mean(parent) > 115
+
+
+def test_robustness_sweep_keeps_absolute_times_of_untouched_fractions():
+    dose, delay = w.PROTOCOL_BMII
+    d, t, nf, labels = w.robustness_sweep(dose, delay)
+    base_times = np.cumsum(delay)
+    assert labels[0] == "base" and nf[0] == 5 and len(labels) == len(nf) == len(d)
+    for row, lab in enumerate(labels):
+        times = np.cumsum(t[row][:nf[row]])
+        assert (t[row][:nf[row]] >= 0).all()
+        if lab.startswith("drop"):
+            j = int(lab[4:])
+            assert np.allclose(times, np.delete(base_times, j)) and np.allclose(d[row][:nf[row]], np.delete(dose, j))
+        elif lab.startswith("shift"):
+            j = int(lab[5])
+            diff = times - base_times
+            assert abs(diff[j]) > 0 and np.allclose(np.delete(diff, j), 0.0)
+    assert sum(l.startswith("drop") for l in labels) == 5 and sum(l.startswith("shift") for l in labels) >= 12
