@@ -412,7 +412,7 @@ def main():
     ap.add_argument("--chains", type=int, default=None)
     ap.add_argument("--reserve-sms", type=int, default=None)
     ap.add_argument("--cluster", type=int, default=None, help="CTAs per simulation of the S2+S3 kernel (1, 2, 4, 8)")
-    ap.add_argument("--oracle-steps", type=int, default=600)
+    ap.add_argument("--oracle-steps", type=int, default=1500, help="CA steps of the oracle sample (about 15 s on one core)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--ga", action="store_true", help="configs[4] streaming + host GA loop at reduced size (probe)")
     ap.add_argument("--ga-population", type=int, default=128)
