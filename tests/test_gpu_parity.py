@@ -333,3 +333,37 @@ def test_dense_starving_tumour_long_window_all_cell_paths_agree():
     r.run(240 / p["steps_per_hour"])
     assert_ints_equal(sa[0][1], r.get_state(), "oracle f32, 240 steps")
     assert_fields_bitwise(sa[0][1], r.get_state(), "oracle f32, 240 steps")
+
+
+@pytest.mark.parametrize("dims", [(3, 3, 3), (4, 4, 3), (6, 8, 3), (64, 64, 3), (64, 4, 5), (4, 64, 4), (96, 4, 3), (8, 68, 4)])
+def test_degenerate_lattices(dims):
+    """Smallest and thinnest lattices: one interior plane, one interior row, a single interior site; a lone cell, then
+    (where there is room) its first divisions.  Integers and fields bit-identical to the fp32 oracle, fp64 within 1e-4."""
+    p = w.stress_params()
+    seed = 31
+    g = _gpu(2, dims, p, max_frac=1)
+    g.seed("single", rng_seed=seed, sim_id_base=7)
+    g.set_protocols(np.array([[1.0], [0.0]]), np.array([[5 / p["steps_per_hour"]], [0.0]]), np.array([1, 0], np.int32))
+    refs = []
+    for b in range(2):
+        pair = []
+        for prec in ("f32", "f64"):
+            r = o.OracleSim(*dims, p, precision=prec)
+            r.seed("single", rng_seed=seed, sim_id=7 + b)
+            if b == 0:
+                r.set_protocol([1.0], [5 / p["steps_per_hour"]])
+            pair.append(r)
+        refs.append(pair)
+    for s in (1, 11, 50, 120):
+        g.run(s / p["steps_per_hour"])
+        for b in range(2):
+            gs = g.get_state(b)
+            for r in refs[b]:
+                r.run(s / p["steps_per_hour"])
+            assert_ints_equal(gs, refs[b][0].get_state(), "f32 sim %d step %d" % (b, s))
+            assert_fields_bitwise(gs, refs[b][0].get_state(), "f32 sim %d step %d" % (b, s))
+            if s <= 50:
+                assert_ints_equal(gs, refs[b][1].get_state(), "f64 sim %d step %d" % (b, s))
+            assert_fields_close(gs, refs[b][1].get_state(), p, 1e-4, "f64 sim %d step %d" % (b, s))
+    assert g.fitness().tolist() == [refs[0][0].fitness(), refs[1][0].fitness()]
+    g.close()
