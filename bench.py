@@ -145,7 +145,11 @@ def bench_config(args):
     """configs[1] (c2) is the headline.  --workload c3s / c4s are REDUCED-BATCH probes of the configs[2] / configs[3]
     lattices (96^3, 80^3: the tiled diffusion kernel), not headline numbers; config.workload says which one ran."""
     if args.workload == "c2":
-        return w.config(2)
+        cfg = dict(w.config(2))
+        if args.tumour_radius is not None:      # probe of the late phase of the job: the same workload started from a larger spheroid
+            cfg["init"] = dict(cfg["init"], radius=float(args.tumour_radius))
+            cfg["name"] += "-r%g" % args.tumour_radius
+        return cfg
     k = 3 if args.workload == "c3s" else 4
     cfg = dict(w.config(k))
     batch = 64 if k == 3 else 96
@@ -352,7 +356,7 @@ def run_ours(args):
     achieved = B_ALG * B * sites * (1.0 / per_stage_launches) / (launch_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": ("k_diffuse_fused" if args.workload == "c2" else "k_diffuse_tiled") + ": diffusion-reaction stage S1, all n_sub sub-steps (%d launch(es) per CA step)" % round(per_stage_launches),
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
-                "launch_ms": launch_ms, "traffic": ncu_traffic_bytes() if args.workload == "c2" else None, "traffic_unit": "bytes/launch (ncu --set full, profiles/)",
+                "launch_ms": launch_ms, "traffic": ncu_traffic_bytes() if (args.workload == "c2" and args.tumour_radius is None) else None, "traffic_unit": "bytes/launch (ncu --set full, profiles/)",
                 "algorithmic_bytes_per_launch": B_ALG * B * sites / per_stage_launches, "stage_share_of_step": stage_ms * S / ms_per_step}
 
     # ---- end to end through the C ABI with HOST buffers: snapshot + protocols up, fitness down, every step
@@ -385,12 +389,12 @@ def run_ours(args):
         line = {"metric": "site_updates_per_s", "value": value, "unit": "site-updates/s", "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-                "config": {"workload": "BASELINE configs[%d]%s: %d sims/GPU x %dx%dx%d lattice, shared spheroid, random protocols" % ({"c2": 1, "c3s": 2, "c4s": 3}[args.workload], "" if args.workload == "c2" else " REDUCED BATCH (probe, not the headline)", B, nx, ny, nz),
+                "config": {"workload": "BASELINE configs[%d]%s: %d sims/GPU x %dx%dx%d lattice, shared spheroid, random protocols" % ({"c2": 1, "c3s": 2, "c4s": 3}[args.workload], ("" if args.workload == "c2" else " REDUCED BATCH (probe, not the headline)") + ("" if args.tumour_radius is None else " STARTED FROM A BALL OF RADIUS %g (late-phase probe, not the headline)" % args.tumour_radius), B, nx, ny, nz),
                            "ca_steps_per_step": S, "n_sub": params["n_sub"], "l2": "working set %.2f GB/GPU > 126 MB L2 (no flush needed)" % (29.0 * B * sites / 1e9),
                            "sharding": "batch over ranks, no collective"},
                 "protocols_per_hour": world * B * 3600.0 / (ms_per_step * 1e-3 / S * (576000 if args.workload == "c4s" else HORIZON_STEPS)),
                 "protocols_per_hour_note": "extrapolated from the timed CA steps at the start of treatment (~3k-cell tumours); the tumours regrow to ~1.6e5 cells by day 30 and the late steps cost more: see full_horizon_measured",
-                "full_horizon_measured": full_horizon_record() if args.workload == "c2" else None,
+                "full_horizon_measured": full_horizon_record() if (args.workload == "c2" and args.tumour_radius is None) else None,
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
                 "fitness_sample": [float(x) for x in fit_host[:4]]}
         print(json.dumps(line))
@@ -414,6 +418,7 @@ def main():
     ap.add_argument("--cluster", type=int, default=None, help="CTAs per simulation of the S2+S3 kernel (1, 2, 4, 8)")
     ap.add_argument("--oracle-steps", type=int, default=1500, help="CA steps of the oracle sample (about 15 s on one core)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--tumour-radius", type=float, default=None, help="c2 only: start from a BALL of this radius instead of 9 (probe of the late, dense phase)")
     ap.add_argument("--ga", action="store_true", help="configs[4] streaming + host GA loop at reduced size (probe)")
     ap.add_argument("--ga-population", type=int, default=128)
     ap.add_argument("--ga-generations", type=int, default=2)
