@@ -421,10 +421,10 @@ __device__ __forceinline__ void cd_winner(CDShared &sh, uint32_t site, int dir, 
 }
 
 // MODE 0: S2 on every cell of simulation b (READY parents are remembered);  MODE 1: S3 detect by rescanning the map.
-// CTA `rank` of `cs` takes the 16-word tiles rank, rank + cs, ... of the simulation's map.  The CTA compacts the non-empty
-// map words; then every WARP takes half words: 128 consecutive sites = 4 trips of 32 coalesced sites, trips whose 4 map
-// bits are clear are skipped.  All loads of the 4 trips are issued before any site is worked on, so a dense tumour costs
-// about two memory round trips per 128 sites and warp; READY parents first look at their six neighbours (most are blocked).
+// CTA `rank` of `cs` takes the 16-word tiles rank, rank + cs, ... of the simulation's map and compacts the non-empty map
+// words; then every WARP takes whole words and every LANE one map bit = 8 consecutive sites: one 8-byte load of their
+// states, one 16-byte load of their clocks, six 16-byte loads of their fields, all issued before the first site is
+// worked on, and at most three vector stores back.  Nothing is loaded for a lane whose bit is clear.
 template <int MODE>
 __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int cur, int b, int rank, int cs, uint32_t step,
                                         const uint32_t *__restrict__ occ_b, uint32_t nblk, CDShared &sh, int *__restrict__ err,
@@ -436,7 +436,7 @@ __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int 
     uint8_t *stb = L.state + sbase;
     uint16_t *ckb = L.clock + sbase, *dmb = L.damage + sbase;
     const float *f0 = L.f[cur][0] + sbase, *f1 = L.f[cur][1] + sbase, *f2 = L.f[cur][2] + sbase;
-    const bool need_dm = (step + 1u) % (uint32_t)P.repair_period == 0u;
+    const bool need_dm = (step + 1u) % (uint32_t)P.repair_period == 0u;      // damage only matters on repair steps [D G11]
     const uint32_t sid = P.sim_id_base + (uint32_t)b;
     for (uint32_t w0 = 0; w0 < nblk; w0 += (uint32_t)(CD_WCAP * cs)) {
         if (tid == 0) sh.nW = 0;
@@ -447,86 +447,79 @@ __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int 
         }
         __syncthreads();
         const uint32_t nW = sh.nW;
-        for (uint32_t wi = warp; wi < 2u * nW; wi += CD_THREADS / 32) {      // half a word (4 trips of 32 sites) per warp and turn
-            const uint32_t w = sh.W[wi >> 1];
-            const uint32_t occh = (occ_b[w] >> (16u * (wi & 1u))) & 0xFFFFu;
-            if (!occh) continue;
-            const uint32_t site0 = w * 256u + 128u * (wi & 1u) + (uint32_t)lane;
-            uint32_t st[4];
-#pragma unroll
-            for (int r = 0; r < 4; ++r) st[r] = ((occh >> (4 * r)) & 0xFu) ? (uint32_t)__ldcg(sb + site0 + 32u * r) : 0u;
+        for (uint32_t wi = warp; wi < nW; wi += CD_THREADS / 32) {
+            const uint32_t w = sh.W[wi];
+            if (!((occ_b[w] >> lane) & 1u)) continue;                         // no cell in my 8 sites
+            const uint32_t site0 = w * 256u + 8u * (uint32_t)lane;
+            const unsigned long long sv = __ldcg(reinterpret_cast<const unsigned long long *>(sb + site0));
             if (MODE == 0) {
                 // Branch-light form of [D S2].  Per step almost every cell only refreshes its mode bits and counts its clock down;
                 // starvation, the end of a countdown and repair are rare and go through cell_update, which recomputes the cell
                 // from its original values (so the two forms cannot disagree).
-                uint32_t ck[4];
-                float fo[4], fg[4], fh[4];
-                uint32_t hit = 0;
+                const uint4 cv = *reinterpret_cast<const uint4 *>(ckb + site0);
+                uint4 dv = make_uint4(0u, 0u, 0u, 0u);
+                if (need_dm) dv = *reinterpret_cast<const uint4 *>(dmb + site0);
+                const float4 oa = *reinterpret_cast<const float4 *>(f0 + site0), ob = *reinterpret_cast<const float4 *>(f0 + site0 + 4);
+                const float4 ga = *reinterpret_cast<const float4 *>(f1 + site0), gb = *reinterpret_cast<const float4 *>(f1 + site0 + 4);
+                const float4 ha = *reinterpret_cast<const float4 *>(f2 + site0), hb = *reinterpret_cast<const float4 *>(f2 + site0 + 4);
+                const float fo[8] = { oa.x, oa.y, oa.z, oa.w, ob.x, ob.y, ob.z, ob.w };
+                const float fg[8] = { ga.x, ga.y, ga.z, ga.w, gb.x, gb.y, gb.z, gb.w };
+                const float fh[8] = { ha.x, ha.y, ha.z, ha.w, hb.x, hb.y, hb.z, hb.w };
+                const uint32_t c32[4] = { cv.x, cv.y, cv.z, cv.w }, d32[4] = { dv.x, dv.y, dv.z, dv.w };
+                uint32_t cn[4] = { cv.x, cv.y, cv.z, cv.w }, dn[4] = { dv.x, dv.y, dv.z, dv.w };
+                unsigned long long sn = sv;
+                bool dm_dirty = false;
 #pragma unroll
-                for (int r = 0; r < 4; ++r) {
-                    const uint32_t kind = st[r] & 7u;
-                    if (kind != CA_EMPTY && kind != CA_WALL) {
-                        const uint32_t i = site0 + 32u * r;
-                        hit |= 1u << r;
-                        ck[r] = ckb[i];
-                        fo[r] = f0[i]; fg[r] = f1[i]; fh[r] = f2[i];
-                    }
-                }
-#pragma unroll
-                for (int r = 0; r < 4; ++r)
-                    if ((hit >> r) & 1u) {
-                        const uint32_t i = site0 + 32u * r;
-                        const uint32_t s0 = st[r], kind = s0 & 7u;
-                        const bool dead = kind == CA_DEAD;
-                        const bool starved = !dead && (fg[r] < P.G_Q || fh[r] > P.H_Q);
-                        const bool prolif = (fg[r] >= P.G_P) && (fh[r] <= P.H_P);
-                        const uint32_t mode = 2u * (uint32_t)(!prolif) + (uint32_t)(!(fo[r] >= P.O_A));
-                        uint32_t s1 = dead ? s0 : ((s0 & ~0x18u) | (mode << 3));
-                        if (!is_parent(s1)) s1 &= ~CA_BLOCKED;               // "blocked" is only remembered while the cell stays a parent (see S3)
-                        const bool tick = dead || (prolif && !(s0 & CA_READY));
-                        const uint32_t c1 = ck[r] - (uint32_t)tick;
-                        uint32_t dmv = 0;
-                        if (need_dm && !dead) dmv = dmb[i];                   // repair steps only (uniform) [D G11]
-                        if (starved || (tick && c1 == 0u) || dmv > 0u) {      // rare: the general state machine
-                            uint32_t s2 = s0, c2 = ck[r], d2 = need_dm ? dmv : 1u;   // off repair steps damage can only change to 0 (death, lysis)
-                            const uint32_t d0 = d2;
-                            cell_update(P, s2, c2, d2, fo[r], fg[r], fh[r], i, step, sid);
-                            if ((s2 & 7u) == CA_EMPTY) *lys_b = 1;               // a site was vacated: blocked parents must look again
-                            if (!is_parent(s2)) s2 &= ~CA_BLOCKED;
-                            if (s2 != s0) stb[i] = (uint8_t)s2;
-                            if (c2 != ck[r]) ckb[i] = (uint16_t)c2;
-                            if (d2 != d0) dmb[i] = (uint16_t)d2;
-                            if (is_parent(s2)) {
-                                const uint32_t slot = atomicAdd(&sh.nP, 1u);
-                                if (slot < CD_PCAP) sh.Pl[slot] = i | ((s2 & CA_BLOCKED) << 24);
-                            }
-                        } else {
-                            if (s1 != s0) stb[i] = (uint8_t)s1;
-                            if (tick) ckb[i] = (uint16_t)c1;
-                            if (is_parent(s1)) {
-                                const uint32_t slot = atomicAdd(&sh.nP, 1u);
-                                if (slot < CD_PCAP) sh.Pl[slot] = i | ((s1 & CA_BLOCKED) << 24);
-                            }
+                for (int k = 0; k < 8; ++k) {
+                    const uint32_t s0 = (uint32_t)(sv >> (8 * k)) & 0xFFu, kind = s0 & 7u;
+                    if (kind == CA_EMPTY || kind == CA_WALL) continue;
+                    const uint32_t i = site0 + (uint32_t)k;
+                    const uint32_t ck0 = (c32[k >> 1] >> (16 * (k & 1))) & 0xFFFFu;
+                    const bool dead = kind == CA_DEAD;
+                    const bool starved = !dead && (fg[k] < P.G_Q || fh[k] > P.H_Q);
+                    const bool prolif = (fg[k] >= P.G_P) && (fh[k] <= P.H_P);
+                    const uint32_t mode = 2u * (uint32_t)(!prolif) + (uint32_t)(!(fo[k] >= P.O_A));
+                    uint32_t s1 = dead ? s0 : ((s0 & ~0x18u) | (mode << 3));
+                    if (!is_parent(s1)) s1 &= ~CA_BLOCKED;                   // "blocked" is only remembered while the cell stays a parent (see S3)
+                    const bool tick = dead || (prolif && !(s0 & CA_READY));
+                    uint32_t c1 = ck0 - (uint32_t)tick;
+                    const uint32_t dm0 = (d32[k >> 1] >> (16 * (k & 1))) & 0xFFFFu;
+                    if (starved || (tick && c1 == 0u) || dm0 > 0u) {          // rare: the general state machine (dm0 is 0 off repair steps)
+                        uint32_t s2 = s0, c2 = ck0, d2 = need_dm ? dm0 : 1u;   // off repair steps damage can only change to 0 (death, lysis)
+                        const uint32_t dref = d2;
+                        cell_update(P, s2, c2, d2, fo[k], fg[k], fh[k], i, step, sid);
+                        if ((s2 & 7u) == CA_EMPTY) *lys_b = 1;               // a site was vacated: blocked parents must look again
+                        if (!is_parent(s2)) s2 &= ~CA_BLOCKED;
+                        s1 = s2; c1 = c2;
+                        if (d2 != dref) {
+                            if (need_dm) { dn[k >> 1] = (dn[k >> 1] & ~(0xFFFFu << (16 * (k & 1)))) | (d2 << (16 * (k & 1))); dm_dirty = true; }
+                            else dmb[i] = (uint16_t)d2;                       // the vector was not loaded: single store of the 0
                         }
                     }
-            } else {
-                uint32_t em[4];
-#pragma unroll
-                for (int r = 0; r < 4; ++r) {
-                    em[r] = 0u;
-                    if (is_parent(st[r]) && !(trust && (st[r] & CA_BLOCKED))) {        // most READY parents are blocked, and known to be
-                        em[r] = empty_mask(sb, site0 + 32u * r, P.nx, P.nx * P.ny);
-                        const uint32_t nb = em[r] ? (st[r] & ~CA_BLOCKED) : (st[r] | CA_BLOCKED);
-                        if (nb != st[r]) L.state[sbase + site0 + 32u * r] = (uint8_t)nb;
+                    sn = (sn & ~(0xFFull << (8 * k))) | ((unsigned long long)s1 << (8 * k));
+                    cn[k >> 1] = (cn[k >> 1] & ~(0xFFFFu << (16 * (k & 1)))) | ((c1 & 0xFFFFu) << (16 * (k & 1)));
+                    if (is_parent(s1)) {
+                        const uint32_t slot = atomicAdd(&sh.nP, 1u);
+                        if (slot < CD_PCAP) sh.Pl[slot] = i | ((s1 & CA_BLOCKED) << 24);
                     }
                 }
-#pragma unroll
-                for (int r = 0; r < 4; ++r)
-                    if (em[r]) {
-                        const uint32_t site = site0 + 32u * r;
-                        const int dir = detect_decide_from(P, sb, site, step, sid, em[r]);
-                        if (dir >= 0) cd_winner(sh, site, dir, err);
-                    }
+                if (sn != sv) *reinterpret_cast<unsigned long long *>(stb + site0) = sn;
+                if (cn[0] != cv.x || cn[1] != cv.y || cn[2] != cv.z || cn[3] != cv.w)
+                    *reinterpret_cast<uint4 *>(ckb + site0) = make_uint4(cn[0], cn[1], cn[2], cn[3]);
+                if (dm_dirty) *reinterpret_cast<uint4 *>(dmb + site0) = make_uint4(dn[0], dn[1], dn[2], dn[3]);
+            } else {
+#pragma unroll 1
+                for (int k = 0; k < 8; ++k) {
+                    const uint32_t st = (uint32_t)(sv >> (8 * k)) & 0xFFu;
+                    if (!is_parent(st) || (trust && (st & CA_BLOCKED))) continue;      // most READY parents are blocked, and known to be
+                    const uint32_t site = site0 + (uint32_t)k;
+                    const uint32_t em = empty_mask(sb, site, P.nx, P.nx * P.ny);
+                    const uint32_t nb = em ? (st & ~CA_BLOCKED) : (st | CA_BLOCKED);
+                    if (nb != st) stb[site] = (uint8_t)nb;
+                    if (!em) continue;
+                    const int dir = detect_decide_from(P, sb, site, step, sid, em);
+                    if (dir >= 0) cd_winner(sh, site, dir, err);
+                }
             }
         }
         __syncthreads();
