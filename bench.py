@@ -174,6 +174,10 @@ def run_full_horizon(args):
     nx, ny, nz = cfg["dims"]
     torch.cuda.set_device(0)
     g = binding.CaBatch(B, nx, ny, nz, params, max_frac=10, device=0)
+    if args.fused is not None:
+        g.set_option("fused", args.fused)
+    if args.cell_path is not None:
+        g.set_option("cell_path", args.cell_path)
     g.seed(rng_seed=cfg["rng_seed"], sim_id_base=0, **cfg["init"])
     g.run(cfg["warmup_h"])
     g.sync()
@@ -191,7 +195,8 @@ def run_full_horizon(args):
             "fitness_min_mean_max": [float(fit.min()), float(fit.mean()), float(fit.max())],
             "live_min_mean_max": [int(cnt[:, 0].min()), float(cnt[:, 0].mean()), int(cnt[:, 0].max())],
             "occupied_min_mean_max": [int(cnt[:, 12].min()), float(cnt[:, 12].mean()), int(cnt[:, 12].max())],
-            "gpu_launches": g.launch_count, "data": "synthetic"}
+            "gpu_launches": g.launch_count, "data": "synthetic", "options": {"fused": args.fused, "cell_path": args.cell_path},
+            "fitness": [float(x) for x in fit], "counts_live": [int(x) for x in cnt[:, 0]], "counts_dead": [int(x) for x in cnt[:, 3]]}
     print(json.dumps(line))
     g.close()
 
@@ -413,6 +418,7 @@ def main():
     ap.add_argument("--workload", default="c2", choices=["c2", "c3s", "c4s"], help="c2 = headline; c3s / c4s = reduced-batch probes of the 96^3 / 80^3 lattices")
     ap.add_argument("--fused", type=int, default=None)
     ap.add_argument("--graph-steps", type=int, default=None)
+    ap.add_argument("--cell-path", type=int, default=None, help="0: generic S2/S3 scan kernels")
     ap.add_argument("--chains", type=int, default=None)
     ap.add_argument("--reserve-sms", type=int, default=None)
     ap.add_argument("--cluster", type=int, default=None, help="CTAs per simulation of the S2+S3 kernel (1, 2, 4, 8)")
