@@ -213,6 +213,10 @@ def run_ga_probe(args):
     torch.cuda.set_device(0)
     B = args.ga_batch
     g = binding.CaBatch(B, nx, ny, nz, params, max_frac=10, device=0)
+    if args.chains is not None:
+        g.set_option("chains", args.chains)
+    if args.reserve_sms is not None:
+        g.set_option("reserve_sms", args.reserve_sms)
     g.seed(rng_seed=cfg["rng_seed"], sim_id_base=0, **cfg["init"])
     g.run(cfg["warmup_h"])
     snap = g.get_state(0)
