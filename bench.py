@@ -152,7 +152,7 @@ def bench_config(args):
         return cfg
     k = 3 if args.workload == "c3s" else 4
     cfg = dict(w.config(k))
-    batch = 64 if k == 3 else 96
+    batch = args.batch if args.batch else (64 if k == 3 else 96)
     cfg["batch"] = batch
     for key in ("dose", "delay", "nfrac"):
         cfg[key] = cfg[key][:batch]
@@ -398,7 +398,7 @@ def run_ours(args):
         line = {"metric": "site_updates_per_s", "value": value, "unit": "site-updates/s", "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-                "config": {"workload": "BASELINE configs[%d]%s: %d sims/GPU x %dx%dx%d lattice, shared spheroid, random protocols" % ({"c2": 1, "c3s": 2, "c4s": 3}[args.workload], ("" if args.workload == "c2" else " REDUCED BATCH (probe, not the headline)") + ("" if args.tumour_radius is None else " STARTED FROM A BALL OF RADIUS %g (late-phase probe, not the headline)" % args.tumour_radius), B, nx, ny, nz),
+                "config": {"workload": "BASELINE configs[%d]%s: %d sims/GPU x %dx%dx%d lattice, shared spheroid, random protocols" % ({"c2": 1, "c3s": 2, "c4s": 3}[args.workload], ("" if args.workload == "c2" else (" FULL BATCH (probe: first steps only, stand-in spheroid)" if B >= (512 if args.workload == "c3s" else 1024) else " REDUCED BATCH (probe, not the headline)")) + ("" if args.tumour_radius is None else " STARTED FROM A BALL OF RADIUS %g (late-phase probe, not the headline)" % args.tumour_radius), B, nx, ny, nz),
                            "ca_steps_per_step": S, "n_sub": params["n_sub"], "l2": "working set %.2f GB/GPU > 126 MB L2 (no flush needed)" % (29.0 * B * sites / 1e9),
                            "sharding": "batch over ranks, no collective"},
                 "protocols_per_hour": world * B * 3600.0 / (ms_per_step * 1e-3 / S * (576000 if args.workload == "c4s" else HORIZON_STEPS)),
@@ -428,6 +428,7 @@ def main():
     ap.add_argument("--cluster", type=int, default=None, help="CTAs per simulation of the S2+S3 kernel (1, 2, 4, 8)")
     ap.add_argument("--oracle-steps", type=int, default=1500, help="CA steps of the oracle sample (about 15 s on one core)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--batch", type=int, default=0, help="c3s / c4s only: batch size of the probe (default 64 / 96; 512 / 1024 = the full configs)")
     ap.add_argument("--tumour-radius", type=float, default=None, help="c2 only: start from a BALL of this radius instead of 9 (probe of the late, dense phase)")
     ap.add_argument("--ga", action="store_true", help="configs[4] streaming + host GA loop at reduced size (probe)")
     ap.add_argument("--ga-population", type=int, default=128)
