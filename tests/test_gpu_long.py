@@ -135,3 +135,27 @@ def test_c3_c4_full_batch_size_window_against_the_oracle(k, batch, dims):
             else:
                 assert_fields_close(gs, r.get_state(), p, 1e-4, "f64 sim %d" % b)
     g.close()
+
+
+def test_c5_sized_batch_4096_sims():
+    """A configs[4]-sized batch (4096 x 64^3 = 1.07e9 sites, 31 GB): first, a middle and the last simulation of a 24-step
+    window against the fp32 oracle -- 64-bit indexing of every kernel at the size the streaming driver uses."""
+    p = w.default_params()
+    cfg = w.config(5)
+    B = 4096
+    g = binding.CaBatch(B, 64, 64, 64, p, max_frac=10)
+    g.seed(rng_seed=cfg["rng_seed"], sim_id_base=0, kind="ball", radius=9.0, shared_init=False)
+    dose = np.tile(np.array([[2.0]]), (B, 1)); delay = np.full((B, 1), 8.0 / p["steps_per_hour"])
+    g.set_protocols(dose, delay)
+    g.step(24)
+    fit = g.fitness()
+    for b in (0, 2049, B - 1):
+        r = o.OracleSim(64, 64, 64, p, precision="f32")
+        r.seed("ball", radius=9.0, rng_seed=cfg["rng_seed"], sim_id=b)
+        r.set_protocol(dose[b], delay[b])
+        r.step(24)
+        gs = g.get_state(b)
+        assert_ints_equal(gs, r.get_state(), "sim %d" % b)
+        assert_fields_bitwise(gs, r.get_state(), "sim %d" % b)
+        assert fit[b] == r.fitness()
+    g.close()
