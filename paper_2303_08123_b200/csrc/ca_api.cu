@@ -397,7 +397,7 @@ int ca_create(ca_ctx **out, int batch, int nx, int ny, int nz, const ca_params *
     c->cell_path = 1;
     {
         int cs = 1;
-        while (cs < 8 && (long long)batch * cs * 2 <= 2ll * c->sms && (n >> 8) / CD_TILE >= 8 * cs) cs *= 2;   // about 2 CTAs per SM (measured best at c2: 4 per simulation), >= 4 planes per CTA
+        while (cs < 8 && (long long)batch * cs * 2 <= 4ll * c->sms && (n >> 8) / CD_TILE >= 8 * cs) cs *= 2;   // up to 4 CTAs of 256 threads per SM (measured best at c2: 8 per simulation), >= 4 planes per CTA
         c->cs = cs;
     }
     c->graph[0] = c->graph[1] = nullptr; c->graph_len[0] = c->graph_len[1] = 0; c->graph_nodes = 0; c->launches = 0;

@@ -395,7 +395,7 @@ __global__ void __launch_bounds__(256) k_occ_map(const uint8_t *__restrict__ sta
     if ((threadIdx.x & 31) == 0 && c8 * 8 < tot) occ[c8 >> 5] = ballot;
 }
 
-constexpr int CD_THREADS = 512;
+constexpr int CD_THREADS = 256;
 constexpr int CD_WCAP = 2048;     // map words examined per round
 constexpr int CD_TILE = 16;       // map words per interleave tile (one 64x64 plane): CTA rank takes tiles rank, rank + cs, ...
 constexpr int CD_WINCAP = 2048;   // winners per CTA and step
@@ -527,7 +527,7 @@ __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int 
 }
 
 // grid = batch * cs CTAs in clusters of cs; phases: bit 0 S2, bit 1 S3 (detect + apply)
-__global__ void __launch_bounds__(CD_THREADS, 2) k_cells_divide(KParams P, Lattice L, int cur, const long long *__restrict__ d_step, int k,
+__global__ void __launch_bounds__(CD_THREADS, 4) k_cells_divide(KParams P, Lattice L, int cur, const long long *__restrict__ d_step, int k,
                                                                 const uint32_t *__restrict__ occ, int cs, int phases, int *__restrict__ err, int b0, int *__restrict__ lys)
 {
     __shared__ CDShared sh;
