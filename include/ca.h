@@ -25,6 +25,12 @@
  *     HOST memory synchronise that stream, the others are asynchronous.
  *   - Lattice arrays are [sim][z][y][x], x fastest; linear site index i = (z*ny + y)*nx + x.
  *     The outermost one-site layer is WALL (Dirichlet medium values, never a cell) [D G2].
+ *   - Every call runs on the device the context was created on and restores the caller's current device.
+ *   - Deferred device errors (CA_EOVERFLOW: more births of one simulation in one step than the winner lists hold,
+ *     i.e. > 2048 per CTA + n/8 per simulation; the surplus births are dropped) are reported by the next call that
+ *     synchronises -- ca_sync, ca_get_state, ca_fitness / ca_counts with HOST output.  With DEVICE output those
+ *     two stay asynchronous: call ca_sync to observe errors.  ca_seed and a whole-batch ca_set_state clear them.
+ *   - Fitness is fp32: exact while the lattice has fewer than 2^24 interior sites (all BASELINE configs).
  *   - There is no CPU fallback: without a CUDA device every compute entry point fails with CA_ECUDA.
  */
 #ifndef CA_B200_H
@@ -89,6 +95,7 @@ size_t ca_workspace_bytes(int batch, int nx, int ny, int nz, int max_frac);
  *   stream     a cudaStream_t; all work of this context runs on it.  NULL: the context creates and owns a
  *              non-blocking stream (the legacy default stream cannot be captured into CUDA graphs).
  * The context is bound to the CUDA device that is current at the time of the call. */
+/* batch <= 65535. */
 int ca_create(ca_ctx **out, int batch, int nx, int ny, int nz, const ca_params *p, int max_frac,
               void *workspace, size_t workspace_bytes, void *stream);
 int ca_destroy(ca_ctx *c);
@@ -108,7 +115,8 @@ int ca_set_rng(ca_ctx *c, uint64_t rng_seed, uint32_t sim_id_base);
  * in whichever ca_run call reaches it; fractions on one step are applied in list order; dose 0 is
  * a legal no-op (the paper's sparse 240-slot vector).  CA_EPROTO (nothing changed)
  * if a dose or delay is negative or not finite, a delay is not a whole number of steps
- * (|delay*steps_per_hour - round| > 1e-6), nfrac[b] is outside 0..max_frac_in, max_frac_in exceeds
+ * (tested to fp32 precision, |delay*steps_per_hour - round| > 4e-7 * max(1, delay*steps_per_hour), because the
+ * ABI takes fp32: 0.35 h arrives as 209.9999964 steps; an accepted delay is snapped to the step grid), nfrac[b] is outside 0..max_frac_in, max_frac_in exceeds
  * the capacity given to ca_create, or some S_bj lies before the current step. */
 int ca_set_protocols(ca_ctx *c, const float *dose_gy, const float *delay_h, const int32_t *nfrac,
                      int max_frac_in, float t0_h);
@@ -116,7 +124,9 @@ int ca_set_protocols(ca_ctx *c, const float *dose_gy, const float *delay_h, cons
 /* Advance every simulation to absolute time t_end_h (step index round(t_end_h*steps_per_hour));
  * one CA step = irradiate, n_sub diffusion-reaction sub-steps, cell state, division [D G15].
  * Asynchronous; ca_run(a); ca_run(b) is bitwise the same as ca_run(b).  CA_ESTATE before
- * ca_seed/ca_set_state, CA_EINVAL if t_end_h lies in the past. */
+ * ca_seed/ca_set_state, CA_EINVAL if t_end_h lies in the past or is not finite.  CA_ECUDA if a kernel of a step
+ * cannot be launched: nothing of that step (or, inside a CUDA graph, of that group of steps) is enqueued and the
+ * step counter stays where it was. */
 int ca_run(ca_ctx *c, double t_end_h);
 /* Same, by step count. */
 int ca_step(ca_ctx *c, int64_t nsteps);
@@ -150,8 +160,7 @@ int ca_stage(ca_ctx *c, int stage, int arg);
  *   "fused"        1 = temporally fused diffusion kernels (default), 0 = one launch per sub-step
  *   "cell_path"    1 = clustered S2+S3 kernel driven by the occupancy map when the lattice allows (default), 0 = generic scans
  *   "cluster"      CTAs per simulation of the clustered kernel: 1, 2, 4 or 8
- *   "chains"       2 = two half-batch chains on forked graph branches (measured slower at configs[1]; default 1)
- *   "reserve_sms"  SMs the diffusion kernel leaves free when chains = 2
+ *   "inject_launch_error"  1 = fault injection: the next step / stage call behaves as if a kernel launch had failed
  * CA_EINVAL on an unknown name or value. */
 int ca_set_option(ca_ctx *c, const char *name, int value);
 /* Number of kernel launches (graph nodes included) issued by this context so far. */

@@ -22,7 +22,7 @@ thread_local std::string g_create_error;
 size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 
 struct Layout {
-    size_t field[2][3], state, clock, damage, occ, lys, winners, nwin, step, err, counts, fitness, fire, dose, nfrac, stage, total;
+    size_t field[2][3], state, clock, damage, occ, lys, winners, nwin, spill_n, step, err, counts, fitness, fire, dose, nfrac, stage, total;
     unsigned int cap;
 };
 
@@ -43,6 +43,7 @@ Layout make_layout(int batch, long long n, int max_frac)
     Y.cap = (unsigned int)cap;
     Y.winners = o; o = align_up(o + cap * 8);
     Y.nwin = o;    o = align_up(o + kMaxGraphSteps * 4);
+    Y.spill_n = o; o = align_up(o + (size_t)batch * 4);
     Y.step = o;    o = align_up(o + 8);
     Y.err = o;     o = align_up(o + 4);
     Y.counts = o;  o = align_up(o + (size_t)batch * CA_NCOUNT * 4);
@@ -84,9 +85,8 @@ struct ca_ctx {
     bool mapped_ok;               // simulations are whole multiples of 256 sites: clustered S2+S3 kernel usable
     int cell_path;                 // option: 1 = clustered S2+S3 kernel when usable, 0 = generic scan kernels
     int cs;                        // CTAs per simulation (cluster size) of the clustered kernel
-    int chains, reserve;           // options: 2 = two concurrent half-batch chains inside a graph; SMs the diffusion kernel leaves free
-    cudaStream_t aux[2];
-    cudaEvent_t ev_fork, ev_join[2];
+    unsigned int *d_spill_n;       // per simulation: winners that did not fit the CTA's shared list (spilled to d_winners)
+    cudaError_t launch_err;        // first failed launch since the last check (launch errors are not sticky: remembered here)
     // options
     int graph_steps;
     int fused;
@@ -111,6 +111,14 @@ int cuda_fail(ca_ctx *c, cudaError_t e, const char *what)
     return fail(c, CA_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
 }
 
+// every entry point runs on the context's device and puts the caller's current device back on return
+struct DeviceGuard {
+    int prev = -1;
+    bool changed = false;
+    explicit DeviceGuard(int dev) { if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) changed = cudaSetDevice(dev) == cudaSuccess; }
+    ~DeviceGuard() { if (changed) cudaSetDevice(prev); }
+};
+
 #define CA_CUDA(c, call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail((c), e_, #call); } while (0)
 
 void drop_graphs(ca_ctx *c)
@@ -119,11 +127,9 @@ void drop_graphs(ca_ctx *c)
         if (c->graph[q]) { cudaGraphExecDestroy(c->graph[q]); c->graph[q] = nullptr; c->graph_len[q] = 0; }
 }
 
-// two concurrent half-batch chains: only on the fast path (fused fixed-size diffusion + clustered S2+S3)
-bool use_chains(const ca_ctx *c)
-{
-    return c->chains == 2 && c->P.batch >= 2 && c->fused && c->fplan.ok && c->fplan.fixed != 0 && c->mapped_ok && c->cell_path;
-}
+// a kernel launch failed: remember the first error (cudaGetLastError clears it) until run_plain / ca_stage reports it
+inline void note_launch(ca_ctx *c, cudaError_t e) { if (e != cudaSuccess && c->launch_err == cudaSuccess) c->launch_err = e; }
+inline void note_last(ca_ctx *c) { note_launch(c, cudaGetLastError()); }
 
 inline unsigned int blocks_for(long long n, int threads) { return (unsigned int)((n + threads - 1) / threads); }
 
@@ -135,14 +141,15 @@ unsigned int scan_grid(const ca_ctx *c)
 }
 
 // S2 and/or S3 through the occupancy map: one cluster of c->cs CTAs per simulation
-void enqueue_cells_divide(ca_ctx *c, int cur, int k, int phases, bool have_map, int b0 = 0, int nb = -1, cudaStream_t st = nullptr)
+void enqueue_cells_divide(ca_ctx *c, int cur, int k, int phases, bool have_map)
 {
-    if (nb < 0) nb = c->P.batch;
-    if (!st) st = c->stream;
+    const int nb = c->P.batch, b0 = 0;
+    cudaStream_t st = c->stream;
     const KParams &P = c->P;
     const long long tot = P.n * P.batch;
     if (!have_map) {
         k_occ_map<<<blocks_for(tot / 8, 256), 256, 0, st>>>(c->L.state, tot, c->d_occ);   // whole batch (cheap; only on the generic paths)
+        note_last(c);
         c->launches += 1;
     }
     cudaLaunchConfig_t cfg = {};
@@ -153,41 +160,46 @@ void enqueue_cells_divide(ca_ctx *c, int cur, int k, int phases, bool have_map, 
     at[0].id = cudaLaunchAttributeClusterDimension;
     at[0].val.clusterDim.x = (unsigned int)c->cs; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
-    cudaLaunchKernelEx(&cfg, k_cells_divide, P, c->L, cur, (const long long *)c->d_step, k, (const uint32_t *)c->d_occ, c->cs, phases, c->d_err, b0, c->d_lys);
+    const SpillArgs sp = { c->d_winners, c->d_spill_n, c->Y.cap / (unsigned int)P.batch };
+    note_launch(c, cudaLaunchKernelEx(&cfg, k_cells_divide, P, c->L, cur, (const long long *)c->d_step, k, (const uint32_t *)c->d_occ, c->cs, phases, c->d_err, b0, c->d_lys, sp));
     c->launches += 1;
 }
 
 // Enqueue the kernels of ONE CA step (without irradiation) at device step *d_step + k, starting from
 // ping-pong buffer `cur`; returns the buffer holding the fields afterwards.   [D G15]
-int enqueue_step(ca_ctx *c, int cur, int k, int b0 = 0, int nb = -1, cudaStream_t st = nullptr, int reserve = 0)
+int enqueue_step(ca_ctx *c, int cur, int k)
 {
     const KParams &P = c->P;
-    if (nb < 0) nb = P.batch;
-    if (!st) st = c->stream;
+    cudaStream_t st = c->stream;
     const long long tot = P.n * P.batch;
     const bool mapped = c->mapped_ok && c->cell_path;
     bool have_map = false;
+    if (c->launch_err != cudaSuccess) return cur;                          // an earlier launch failed: enqueue nothing on top of it
     if (c->fused && fused_supported(c->fplan)) {
         cudaError_t fe;
-        const int np = launch_fused(c->fplan, c->L, cur, mapped ? c->d_occ : nullptr, st, &fe, b0, nb, reserve);   // S1: all n_sub sub-steps, one pass over HBM (two if n_sub > 4)
+        const int np = launch_fused(c->fplan, c->L, cur, mapped ? c->d_occ : nullptr, st, &fe);   // S1: all n_sub sub-steps, one pass over HBM (two if n_sub > 4)
+        note_launch(c, fe);                                                // a failed pass leaves `cur` where it was; the caller stops on launch_err
         if (np & 1) cur ^= 1;
         c->launches += np;
-        have_map = mapped && c->fplan.fixed != 0;
+        have_map = mapped && c->fplan.writes_map;
     } else {
         for (int m = 0; m < P.n_sub; ++m) {                                // S1, one launch per sub-step
             k_diffuse_sub<<<blocks_for(tot, 256), 256, 0, c->stream>>>(P, c->L, cur);
+            note_last(c);
             cur ^= 1;
         }
         c->launches += P.n_sub;
     }
+    if (c->launch_err != cudaSuccess) return cur;                          // S1 did not start: S2/S3 must not run on undiffused fields
     if (mapped) {
-        enqueue_cells_divide(c, cur, k, 3, have_map, b0, nb, st);           // S2 + S3 in one clustered launch
+        enqueue_cells_divide(c, cur, k, 3, have_map);                       // S2 + S3 in one clustered launch
         return cur;
     }
     const ScanArgs sa = { c->d_winners, c->d_nwin + k, c->Y.cap, c->d_err };
     k_scan<0><<<scan_grid(c), 256, 0, c->stream>>>(P, c->L, cur, c->d_step, k, sa);                            // S2
     k_scan<1><<<scan_grid(c), 256, 0, c->stream>>>(P, c->L, cur, c->d_step, k, sa);                            // S3 detect
     k_div_apply<<<64, 128, 0, c->stream>>>(P, c->L, c->d_step, k, c->d_winners, c->d_nwin + k, c->Y.cap);
+    note_last(c);
     c->launches += 3;
     return cur;
 }
@@ -197,6 +209,7 @@ int enqueue_irradiate(ca_ctx *c)
     const KParams &P = c->P;
     dim3 grid(std::min<unsigned int>(blocks_for(P.n, 256), 512u), (unsigned int)P.batch);
     k_irradiate<<<grid, 256, 0, c->stream>>>(P, c->L, c->cur, c->d_fire, c->d_dose, c->d_nfrac, c->max_frac, c->d_step, 0);
+    note_last(c);
     c->launches += 1;
     return 0;
 }
@@ -220,24 +233,14 @@ int run_plain(ca_ctx *c, long long nsteps)
             const long long before = c->launches;
             CA_CUDA(c, cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
             int cur = par;
-            if (use_chains(c)) {
-                // Two half-batches on two forked streams.  Simulations never interact, so the halves are independent
-                // chains; while one half is in its latency-bound S2+S3 kernel the other half's diffusion kernel fills
-                // the machine (it leaves c->reserve SMs free so that those CTAs find a home at once).
-                const int half = c->P.batch / 2;
-                CA_CUDA(c, cudaEventRecord(c->ev_fork, c->stream));
-                for (int ch = 0; ch < 2; ++ch) {
-                    CA_CUDA(c, cudaStreamWaitEvent(c->aux[ch], c->ev_fork, 0));
-                    cur = par;
-                    for (int k = 0; k < G; ++k) cur = enqueue_step(c, cur, k, ch * half, ch ? c->P.batch - half : half, c->aux[ch], c->reserve);
-                    CA_CUDA(c, cudaEventRecord(c->ev_join[ch], c->aux[ch]));
-                    CA_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_join[ch], 0));
-                }
-            } else {
-                for (int k = 0; k < G; ++k) cur = enqueue_step(c, cur, k);
-            }
+            for (int k = 0; k < G; ++k) cur = enqueue_step(c, cur, k);
             enqueue_advance(c, G);
             cudaError_t e = cudaStreamEndCapture(c->stream, &g);
+            if (c->launch_err != cudaSuccess) {                              // a kernel of the step could not be launched: no graph, no run
+                if (e == cudaSuccess) cudaGraphDestroy(g);
+                const cudaError_t le = c->launch_err; c->launch_err = cudaSuccess; c->launches = before;
+                return cuda_fail(c, le, "kernel launch (graph capture)");
+            }
             if (e != cudaSuccess) return cuda_fail(c, e, "cudaStreamEndCapture");
             if (cur != par) { cudaGraphDestroy(g); return fail(c, CA_EINVAL, "graph_steps * swaps must be even"); }
             e = cudaGraphInstantiate(&c->graph[par], g, 0);
@@ -253,7 +256,12 @@ int run_plain(ca_ctx *c, long long nsteps)
         nsteps -= G;
     }
     while (nsteps > 0) {
-        c->cur = enqueue_step(c, c->cur, 0);
+        const int nxt = enqueue_step(c, c->cur, 0);
+        if (c->launch_err != cudaSuccess) {                                  // stop at once: S2/S3 must not run on undiffused fields
+            const cudaError_t le = c->launch_err; c->launch_err = cudaSuccess;
+            return cuda_fail(c, le, "kernel launch");
+        }
+        c->cur = nxt;
         enqueue_advance(c, 1);
         c->step += 1;
         nsteps -= 1;
@@ -266,7 +274,7 @@ int run_steps(ca_ctx *c, long long nsteps)
 {
     if (!c->seeded) return fail(c, CA_ESTATE, "ca_run before ca_seed / ca_set_state");
     if (nsteps < 0) return fail(c, CA_EINVAL, "target time lies in the past");
-    CA_CUDA(c, cudaSetDevice(c->device));
+    DeviceGuard guard_(c->device);
     const long long end = c->step + nsteps;
     while (c->step < end) {
         // next step >= c->step on which some fraction fires (host knows the whole schedule)
@@ -328,6 +336,7 @@ int ca_create(ca_ctx **out, int batch, int nx, int ny, int nz, const ca_params *
 {
     if (!out) return fail(nullptr, CA_EINVAL, "out is NULL");
     *out = nullptr;
+    if (batch > 65535) return fail(nullptr, CA_EINVAL, "batch must be <= 65535 (one grid row per simulation in the per-simulation kernels)");
     if (!p || batch < 1 || nx < 3 || ny < 3 || nz < 3) return fail(nullptr, CA_EINVAL, "bad batch / lattice dims (each dim >= 3)");
     if (max_frac < 1 || max_frac > 64) return fail(nullptr, CA_EINVAL, "max_frac must be 1..64");
     if (p->n_sub < 1 || p->n_sub > 8 || p->steps_per_hour < 1) return fail(nullptr, CA_EINVAL, "n_sub must be 1..8, steps_per_hour >= 1");
@@ -367,6 +376,8 @@ int ca_create(ca_ctx **out, int batch, int nx, int ny, int nz, const ca_params *
     c->L.damage = (uint16_t *)(c->ws + c->Y.damage);
     c->d_winners = (unsigned long long *)(c->ws + c->Y.winners);
     c->d_nwin = (unsigned int *)(c->ws + c->Y.nwin);
+    c->d_spill_n = (unsigned int *)(c->ws + c->Y.spill_n);
+    c->launch_err = cudaSuccess;
     c->d_step = (long long *)(c->ws + c->Y.step);
     c->d_err = (int *)(c->ws + c->Y.err);
     c->d_counts = (int *)(c->ws + c->Y.counts);
@@ -379,6 +390,7 @@ int ca_create(ca_ctx **out, int batch, int nx, int ny, int nz, const ca_params *
     c->d_lys = (int *)(c->ws + c->Y.lys);
     c->stream = (cudaStream_t)stream;
     c->own_stream = false;
+    DeviceGuard guard_(dev);
     if (!c->stream) {                     // the legacy default stream cannot be captured into CUDA graphs
         e = cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking);
         if (e != cudaSuccess) { int rc = cuda_fail(nullptr, e, "cudaStreamCreateWithFlags"); delete c; return rc; }
@@ -391,9 +403,6 @@ int ca_create(ca_ctx **out, int batch, int nx, int ny, int nz, const ca_params *
     c->fire.assign((size_t)batch * max_frac, 0); c->dose.assign((size_t)batch * max_frac, 0.0f); c->nfrac.assign(batch, 0);
     c->graph_steps = 20; c->fused = 1;
     c->mapped_ok = (n % 256 == 0) && n < (1ll << 29);
-    c->chains = 1; c->reserve = 4;   // two chains measured SLOWER at c2 (137-148 vs 132 us/step): kept as an option only
-    for (int q = 0; q < 2; ++q) { cudaStreamCreateWithFlags(&c->aux[q], cudaStreamNonBlocking); cudaEventCreateWithFlags(&c->ev_join[q], cudaEventDisableTiming); }
-    cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming);
     c->cell_path = 1;
     {
         int cs = 1;
@@ -413,10 +422,9 @@ int ca_create(ca_ctx **out, int batch, int nx, int ny, int nz, const ca_params *
 int ca_destroy(ca_ctx *c)
 {
     if (!c) return CA_OK;
+    DeviceGuard guard_(c->device);
     cudaStreamSynchronize(c->stream);
     drop_graphs(c);
-    for (int q = 0; q < 2; ++q) { cudaStreamDestroy(c->aux[q]); cudaEventDestroy(c->ev_join[q]); }
-    cudaEventDestroy(c->ev_fork);
     if (c->own_stream) cudaStreamDestroy(c->stream);
     delete c;
     return CA_OK;
@@ -434,7 +442,7 @@ int ca_seed(ca_ctx *c, const ca_init *init, uint64_t rng_seed, uint32_t sim_id_b
 {
     if (!c || !init) return CA_EINVAL;
     if (init->kind < 0 || init->kind > 2) return fail(c, CA_EINVAL, "unknown init kind");
-    CA_CUDA(c, cudaSetDevice(c->device));
+    DeviceGuard guard_(c->device);
     ca_set_rng(c, rng_seed, sim_id_base);
     const long long tot = c->P.n * c->P.batch;
     k_seed<<<blocks_for(tot, 256), 256, 0, c->stream>>>(c->P, c->L, *init);
@@ -463,8 +471,11 @@ int ca_set_protocols(ca_ctx *c, const float *dose_gy, const float *delay_h, cons
             const double d = (double)dose_gy[(size_t)b * max_frac_in + j], dl = (double)delay_h[(size_t)b * max_frac_in + j];
             if (!(d >= 0.0) || !(dl >= 0.0) || !std::isfinite(d) || !std::isfinite(dl)) return fail(c, CA_EPROTO, "negative or non-finite dose / delay");
             const double ds = dl * sph;
-            if (std::fabs(ds - std::floor(ds + 0.5)) > 1e-6) return fail(c, CA_EPROTO, "delay is not a whole number of CA steps");
-            t += dl;
+            // the ABI takes fp32 delays: a step-aligned delay such as 0.35 h or 6.1 h arrives as 209.9999964 / 3659.99994 steps,
+            // so alignment is tested to fp32 precision and the delay is snapped to the step grid before it is accumulated
+            const double dsr = std::floor(ds + 0.5);
+            if (std::fabs(ds - dsr) > 4e-7 * std::max(1.0, ds)) return fail(c, CA_EPROTO, "delay is not a whole number of CA steps");
+            t += dsr / sph;
             const double S = std::floor(t * sph + 0.5);                     // [D G24]
             if (S < (double)c->step) return fail(c, CA_EPROTO, "fraction scheduled before the current step");
             if (S > 2.0e9) return fail(c, CA_EPROTO, "fraction scheduled beyond 2e9 steps");
@@ -475,7 +486,7 @@ int ca_set_protocols(ca_ctx *c, const float *dose_gy, const float *delay_h, cons
     }
     std::sort(all.begin(), all.end());
     all.erase(std::unique(all.begin(), all.end()), all.end());
-    CA_CUDA(c, cudaSetDevice(c->device));
+    DeviceGuard guard_(c->device);
     CA_CUDA(c, cudaStreamSynchronize(c->stream));                           // host vectors below are re-used as copy sources
     c->fire.swap(fire); c->dose.swap(dose); c->nfrac.assign(nfrac, nfrac + B); c->fire_sorted.swap(all);
     CA_CUDA(c, cudaMemcpyAsync(c->d_fire, c->fire.data(), (size_t)B * F * 4, cudaMemcpyHostToDevice, c->stream));
@@ -494,6 +505,7 @@ int ca_step(ca_ctx *c, int64_t nsteps)
 int ca_run(ca_ctx *c, double t_end_h)
 {
     if (!c) return CA_EINVAL;
+    if (!std::isfinite(t_end_h) || std::fabs(t_end_h) * (double)c->hp.steps_per_hour > 4.0e18) return fail(c, CA_EINVAL, "t_end_h is not a finite, representable time");
     const long long end = (long long)std::floor(t_end_h * (double)c->hp.steps_per_hour + 0.5);
     return run_steps(c, end - c->step);
 }
@@ -508,7 +520,7 @@ int ca_get_step(ca_ctx *c, int64_t *step)
 int ca_sync(ca_ctx *c)
 {
     if (!c) return CA_EINVAL;
-    CA_CUDA(c, cudaSetDevice(c->device));
+    DeviceGuard guard_(c->device);
     return check_deferred(c);
 }
 
@@ -516,7 +528,7 @@ int ca_counts(ca_ctx *c, int32_t *out, int out_is_device)
 {
     if (!c || !out) return CA_EINVAL;
     if (!c->seeded) return fail(c, CA_ESTATE, "ca_counts before ca_seed / ca_set_state");
-    CA_CUDA(c, cudaSetDevice(c->device));
+    DeviceGuard guard_(c->device);
     int rc = enqueue_counts(c);
     if (rc) return rc;
     const size_t bytes = (size_t)c->P.batch * CA_NCOUNT * 4;
@@ -528,7 +540,7 @@ int ca_fitness(ca_ctx *c, float *out, int out_is_device)
 {
     if (!c || !out) return CA_EINVAL;
     if (!c->seeded) return fail(c, CA_ESTATE, "ca_fitness before ca_seed / ca_set_state");
-    CA_CUDA(c, cudaSetDevice(c->device));
+    DeviceGuard guard_(c->device);
     int rc = enqueue_counts(c);
     if (rc) return rc;
     const size_t bytes = (size_t)c->P.batch * 4;
@@ -539,7 +551,7 @@ int ca_fitness(ca_ctx *c, float *out, int out_is_device)
 int ca_get_state(ca_ctx *c, int sim, uint8_t *state, uint16_t *clock, uint16_t *damage, float *o2, float *glc, float *h, int64_t *step)
 {
     if (!c || sim < 0 || sim >= c->P.batch) return c ? fail(c, CA_EINVAL, "sim out of range") : CA_EINVAL;
-    CA_CUDA(c, cudaSetDevice(c->device));
+    DeviceGuard guard_(c->device);
     const size_t n = (size_t)c->P.n, o = (size_t)sim * n;
     if (state)  CA_CUDA(c, cudaMemcpyAsync(state, c->L.state + o, n, cudaMemcpyDeviceToHost, c->stream));
     if (clock)  CA_CUDA(c, cudaMemcpyAsync(clock, c->L.clock + o, n * 2, cudaMemcpyDeviceToHost, c->stream));
@@ -567,7 +579,7 @@ int ca_set_state(ca_ctx *c, int sim_first, int sim_count, const uint8_t *state, 
             if (wall != ((s & 7) == CA_WALL) || (s & 7) == 6 || (s & 0x80)) return fail(c, CA_EINVAL, "state: WALL layer misplaced or invalid code");
         }
     }
-    CA_CUDA(c, cudaSetDevice(c->device));
+    DeviceGuard guard_(c->device);
     const size_t n = (size_t)P.n;
     struct Item { const void *src; uint8_t *base; size_t elem; };
     const Item items[] = {
@@ -590,6 +602,8 @@ int ca_set_state(ca_ctx *c, int sim_first, int sim_count, const uint8_t *state, 
         c->step = (long long)step;
         CA_CUDA(c, cudaMemcpyAsync(c->d_step, &c->step, 8, cudaMemcpyHostToDevice, c->stream));
     }
+    if (state && sim_first == 0 && sim_count == P.batch) CA_CUDA(c, cudaMemsetAsync(c->d_err, 0, 4, c->stream));   // a whole new batch: deferred errors of the old one are gone
+    if (state) CA_CUDA(c, cudaMemsetAsync(c->d_lys + sim_first, 1, (size_t)sim_count * 4, c->stream));             // no "blocked" mark of the old lattice can be trusted
     CA_CUDA(c, cudaStreamSynchronize(c->stream));      // the caller's arrays may be pageable: do not return before they are consumed
     c->seeded = true;
     return CA_OK;
@@ -599,15 +613,17 @@ int ca_stage(ca_ctx *c, int stage, int arg)
 {
     if (!c) return CA_EINVAL;
     if (!c->seeded) return fail(c, CA_ESTATE, "ca_stage before ca_seed / ca_set_state");
-    CA_CUDA(c, cudaSetDevice(c->device));
+    DeviceGuard guard_(c->device);
     const KParams &P = c->P;
     const long long tot = P.n * P.batch;
+    if (c->launch_err != cudaSuccess) { const cudaError_t le = c->launch_err; c->launch_err = cudaSuccess; return cuda_fail(c, le, "kernel launch"); }
     switch (stage) {
     case 0: enqueue_irradiate(c); break;
     case 1:
         if (c->fused && fused_supported(c->fplan)) {
             cudaError_t fe;
             const int np = launch_fused(c->fplan, c->L, c->cur, nullptr, c->stream, &fe);
+            if (fe != cudaSuccess) return cuda_fail(c, fe, "diffusion kernel launch");   // nothing flipped: a failed pass is never counted
             if (np & 1) c->cur ^= 1;
             c->launches += np;
         }
@@ -631,6 +647,7 @@ int ca_stage(ca_ctx *c, int stage, int arg)
         break;
     default: return fail(c, CA_EINVAL, "unknown stage");
     }
+    if (c->launch_err != cudaSuccess) { const cudaError_t le = c->launch_err; c->launch_err = cudaSuccess; return cuda_fail(c, le, "kernel launch"); }
     CA_CUDA(c, cudaGetLastError());
     return CA_OK;
 }
@@ -643,13 +660,8 @@ int ca_set_option(ca_ctx *c, const char *name, int value)
         c->graph_steps = value; drop_graphs(c); return CA_OK;
     }
     if (!std::strcmp(name, "fused")) { c->fused = value ? 1 : 0; drop_graphs(c); return CA_OK; }
-    if (!std::strcmp(name, "chains")) {
-        if (value != 1 && value != 2) return fail(c, CA_EINVAL, "chains must be 1 or 2");
-        c->chains = value; drop_graphs(c); return CA_OK;
-    }
-    if (!std::strcmp(name, "reserve_sms")) {
-        if (value < 0 || value > 64) return fail(c, CA_EINVAL, "reserve_sms must be 0..64");
-        c->reserve = value; drop_graphs(c); return CA_OK;
+    if (!std::strcmp(name, "inject_launch_error")) {                          // fault injection for the tests: the next step sees a failed kernel launch
+        c->launch_err = value ? cudaErrorLaunchOutOfResources : cudaSuccess; return CA_OK;
     }
     if (!std::strcmp(name, "cluster")) {
         if (value != 1 && value != 2 && value != 4 && value != 8) return fail(c, CA_EINVAL, "cluster must be 1, 2, 4 or 8");

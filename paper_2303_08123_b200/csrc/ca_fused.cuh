@@ -516,9 +516,14 @@ struct FusedPlan {
     bool ok = false;
     int lrp = 0, sms = 0, fixed = 0;   // fixed: 0 run-time dims, 32 / 64: the cubic fast instantiations
     bool tiled = false;                // planes wider than 64 sites: k_diffuse_tiled
+    bool writes_map = false;           // the kernel writes the S2/S3 occupancy map while the state planes pass through it
     int tile_warps = 0;
     FusedArgs args{};
     int npass = 0, pass_nl[2] = { 0, 0 };
+    // per context (= per device and host thread): shared-memory opt-in done, and the last split table, by NL
+    bool attr_done[F_MAXNL + 1] = { false, false, false, false, false };
+    int split_key[F_MAXNL + 1][3] = { { -1, -1, -1 }, { -1, -1, -1 }, { -1, -1, -1 }, { -1, -1, -1 }, { -1, -1, -1 } };
+    int split[F_MAXNL + 1][F_MAXGRID + 1];
 };
 
 inline size_t fused_smem(int nx, int ny, int nl, int lrp, FusedGeom &G)
@@ -540,7 +545,7 @@ inline size_t fused_smem(int nx, int ny, int nl, int lrp, FusedGeom &G)
 // empty lead-in iterations are skipped).  Costs in units of one steady iteration, fitted to the measured kernel.
 inline void fused_split(int units, int nzi, int nl, int grid, int *start)
 {
-    static const double f = getenv("CA_RAMP") ? atof(getenv("CA_RAMP")) : 0.55;
+    const double f = 0.55;                             // cost of one pipeline-fill iteration relative to a steady one (fitted on the B200)
     const double r_wall = f * (2 * nl - 3), r_cut = f * (2 * nl);
     const long long total = (long long)units * nzi;
     double lo = 0.0, hi = (double)total + (double)(units + grid) * r_cut + 1.0;
@@ -577,34 +582,36 @@ inline void fused_split(int units, int nzi, int nl, int grid, int *start)
     for (int g = grid - 1; g >= 0 && start[g] > start[grid]; --g) start[g] = start[grid];
 }
 
+// the split depends on (units, planes, NL, grid) only: the plan keeps the last one per NL
+inline void fused_split_cached(FusedPlan &F, int units, int nzi, int nl, int grid, int *start)
+{
+    int *key = F.split_key[nl];
+    if (key[0] != units || key[1] != nzi || key[2] != grid) {
+        fused_split(units, nzi, nl, grid, F.split[nl]);
+        key[0] = units; key[1] = nzi; key[2] = grid;
+    }
+    memcpy(start, F.split[nl], sizeof(int) * (grid + 1));
+}
+
 template <int NL, int LRP, int NX, int NY>
-inline cudaError_t fused_launch_t(const FusedArgs &A, int grid, cudaStream_t st)
+inline cudaError_t fused_launch_t(FusedPlan &F, const FusedArgs &A, int grid, cudaStream_t st)
 {
     FusedGeom G{};
     fused_smem(A.nx, A.ny, NL, LRP, G);
     G.total_planes = (long long)A.batch * 3 * (A.nz - 2);
     if (grid > F_MAXGRID) grid = F_MAXGRID;
-    {   // the split depends on (units, planes, NL, grid) only: keep the last one
-        static int key[4] = { -1, -1, -1, -1 };
-        static int cached[F_MAXGRID + 1];
-        if (key[0] != A.batch || key[1] != A.nz || key[2] != NL || key[3] != grid) {
-            fused_split(A.batch * 3, A.nz - 2, NL, grid, cached);
-            key[0] = A.batch; key[1] = A.nz; key[2] = NL; key[3] = grid;
-        }
-        memcpy(G.start, cached, sizeof(int) * (grid + 1));
-    }
-    static bool attr_done = false;      // per instantiation
-    if (!attr_done) {
+    fused_split_cached(F, A.batch * 3, A.nz - 2, NL, grid, G.start);
+    if (!F.attr_done[NL]) {            // the opt-in is per device: kept per context, not per process
         cudaError_t e = cudaFuncSetAttribute(k_diffuse_fused<NL, LRP, NX, NY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        F.attr_done[NL] = true;
     }
     k_diffuse_fused<NL, LRP, NX, NY><<<grid, G.nwarps * 32, G.smem_bytes, st>>>(A, G);
     return cudaGetLastError();
 }
 
 template <int NL, int NXG, int NYG>
-inline cudaError_t fused_launch_tiled_t(const FusedPlan &F, const FusedArgs &A, int grid, cudaStream_t st)
+inline cudaError_t fused_launch_tiled_t(FusedPlan &F, const FusedArgs &A, int grid, cudaStream_t st)
 {
     FusedGeom G{};
     fused_smem(64, 64, NL, 32, G);
@@ -612,27 +619,18 @@ inline cudaError_t fused_launch_tiled_t(const FusedPlan &F, const FusedArgs &A, 
     const int units = A.batch * 3 * A.ntx * A.nty;
     G.total_planes = (long long)units * (A.nz - 2);
     if (grid > F_MAXGRID) grid = F_MAXGRID;
-    {
-        static int key[4] = { -1, -1, -1, -1 };
-        static int cached[F_MAXGRID + 1];
-        if (key[0] != units || key[1] != A.nz || key[2] != NL || key[3] != grid) {
-            fused_split(units, A.nz - 2, NL, grid, cached);
-            key[0] = units; key[1] = A.nz; key[2] = NL; key[3] = grid;
-        }
-        memcpy(G.start, cached, sizeof(int) * (grid + 1));
-    }
-    static bool attr_done = false;
-    if (!attr_done) {
+    fused_split_cached(F, units, A.nz - 2, NL, grid, G.start);
+    if (!F.attr_done[NL]) {
         cudaError_t e = cudaFuncSetAttribute(k_diffuse_tiled<NL, NXG, NYG>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        F.attr_done[NL] = true;
     }
     k_diffuse_tiled<NL, NXG, NYG><<<grid, G.nwarps * 32, G.smem_bytes, st>>>(A, G);
     return cudaGetLastError();
 }
 
 template <int NL>
-inline cudaError_t fused_launch_tiled(const FusedPlan &F, const FusedArgs &A, int grid, cudaStream_t st)
+inline cudaError_t fused_launch_tiled(FusedPlan &F, const FusedArgs &A, int grid, cudaStream_t st)
 {
     if (A.nx == 96 && A.ny == 96) return fused_launch_tiled_t<NL, 96, 96>(F, A, grid, st);    // BASELINE configs[2]
     if (A.nx == 80 && A.ny == 80) return fused_launch_tiled_t<NL, 80, 80>(F, A, grid, st);    // BASELINE configs[3]
@@ -656,13 +654,13 @@ inline int fused_tiles(int n, short *t0, short *t1, short *o0, short *o1)
 }
 
 template <int NL>
-inline cudaError_t fused_launch_nl(const FusedPlan &F, const FusedArgs &A, int grid, cudaStream_t st)
+inline cudaError_t fused_launch_nl(FusedPlan &F, const FusedArgs &A, int grid, cudaStream_t st)
 {
     if (F.tiled) return fused_launch_tiled<NL>(F, A, grid, st);
-    if (F.fixed == 64) return fused_launch_t<NL, 32, 64, 64>(A, grid, st);
-    if (F.fixed == 32) return fused_launch_t<NL, 16, 32, 32>(A, grid, st);
-    if (F.lrp == 16) return fused_launch_t<NL, 16, 0, 0>(A, grid, st);
-    return fused_launch_t<NL, 32, 0, 0>(A, grid, st);
+    if (F.fixed == 64) return fused_launch_t<NL, 32, 64, 64>(F, A, grid, st);
+    if (F.fixed == 32) return fused_launch_t<NL, 16, 32, 32>(F, A, grid, st);
+    if (F.lrp == 16) return fused_launch_t<NL, 16, 0, 0>(F, A, grid, st);
+    return fused_launch_t<NL, 32, 0, 0>(F, A, grid, st);
 }
 
 // Decide whether the fused kernel covers this lattice, and precompute its arguments.
@@ -682,6 +680,7 @@ inline void fused_configure(const KParams &P, FusedPlan &F)
     } else if (P.nx % 2 || (P.nx * P.ny) % 16) return;
     F.lrp = P.nx <= 32 ? 16 : 32;
     F.fixed = (P.nx == 64 && P.ny == 64) ? 64 : (P.nx == 32 && P.ny == 32) ? 32 : 0;
+    F.writes_map = F.fixed != 0 && !F.tiled;
     FusedGeom G{};
     if (!F.tiled && (fused_smem(P.nx, P.ny, F_MAXNL, F.lrp, G) > 227 * 1024 || G.nwarps > 16)) return;
     int dev = 0;
@@ -707,25 +706,24 @@ inline void fused_configure(const KParams &P, FusedPlan &F)
 inline bool fused_supported(const FusedPlan &F) { return F.ok; }
 
 // Enqueue all n_sub sub-steps starting from ping-pong buffer `cur`; returns the number of passes (= buffer flips).
-// Simulations [b0, b0 + nb) only (nb < 0: all); `reserve` SMs are left free for a concurrent chain's S2+S3 kernel.
-inline int launch_fused(FusedPlan &F, const Lattice &L, int cur, uint32_t *occ, cudaStream_t st, cudaError_t *err,
-                        int b0 = 0, int nb = -1, int reserve = 0)
+// A failed launch stops the sequence: *err says why, and the return value counts only the passes that were launched.
+inline int launch_fused(FusedPlan &F, const Lattice &L, int cur, uint32_t *occ, cudaStream_t st, cudaError_t *err)
 {
-    if (nb < 0) nb = F.args.batch;
-    const size_t soff = (size_t)b0 * (size_t)F.args.nx * F.args.ny * F.args.nz;
+    const int nb = F.args.batch;
+    const size_t soff = 0;
     *err = cudaSuccess;
     for (int ps = 0; ps < F.npass; ++ps) {
         FusedArgs A = F.args;
         A.batch = nb;
         for (int s = 0; s < 3; ++s) { A.src[s] = L.f[cur][s] + soff; A.dst[s] = L.f[cur ^ 1][s] + soff; }
         A.state = L.state + soff;
-        A.occ = (F.fixed && ps == F.npass - 1 && occ) ? occ + soff / 256 : nullptr;          // the state does not change between passes: write the map once
+        A.occ = (F.writes_map && ps == F.npass - 1 && occ) ? occ + soff / 256 : nullptr;          // the state does not change between passes: write the map once
         FusedGeom G{};
         // CTAs per SM: the 512-thread (nx > 32) kernel fills an SM; smaller lattices use several CTAs per SM
         fused_smem(A.nx, A.ny, F.pass_nl[ps], F.lrp, G);
         const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(std::min<size_t>(4, (227 * 1024) / (G.smem_bytes + 1024)), 512 / (G.nwarps * 32)));
         const long long total = (long long)A.batch * 3 * (A.nz - 2);
-        const int grid = (int)std::max<long long>(1, std::min<long long>((long long)std::max(1, F.sms - reserve) * per_sm, total / 2 + 1));
+        const int grid = (int)std::max<long long>(1, std::min<long long>((long long)F.sms * per_sm, total / 2 + 1));
         cudaError_t e;
         switch (F.pass_nl[ps]) {
         case 1: e = fused_launch_nl<1>(F, A, grid, st); break;

@@ -413,10 +413,20 @@ __device__ __forceinline__ void cluster_sync_all()
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
 
-__device__ __forceinline__ void cd_winner(CDShared &sh, uint32_t site, int dir, int *err)
+// winners beyond the CTA's shared list go to the simulation's slice of the global winners array; only when that is full too
+// (more than n/8 births of one simulation in one step) a birth is dropped, and then the deferred error says so
+struct SpillArgs {
+    unsigned long long *list;     // [batch][cap_per_sim]
+    unsigned int *n;              // [batch]
+    unsigned int cap_per_sim;
+};
+
+__device__ __forceinline__ void cd_winner(CDShared &sh, uint32_t site, int dir, int *err, const SpillArgs &sp, int b)
 {
     const uint32_t slot = atomicAdd(&sh.nwin, 1u);                                  // order is irrelevant to the result
-    if (slot < CD_WINCAP) sh.win[slot] = (site << 3) | (uint32_t)dir;
+    if (slot < CD_WINCAP) { sh.win[slot] = (site << 3) | (uint32_t)dir; return; }
+    const unsigned int g = atomicAdd(sp.n + b, 1u);
+    if (g < sp.cap_per_sim) sp.list[(size_t)b * sp.cap_per_sim + g] = ((unsigned long long)site << 3) | (unsigned long long)dir;
     else *err = CA_EOVERFLOW;
 }
 
@@ -428,7 +438,7 @@ __device__ __forceinline__ void cd_winner(CDShared &sh, uint32_t site, int dir, 
 template <int MODE>
 __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int cur, int b, int rank, int cs, uint32_t step,
                                         const uint32_t *__restrict__ occ_b, uint32_t nblk, CDShared &sh, int *__restrict__ err,
-                                        int *__restrict__ lys_b, bool trust)
+                                        int *__restrict__ lys_b, bool trust, const SpillArgs &sp)
 {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const long long sbase = (long long)b * P.n;
@@ -518,7 +528,7 @@ __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int 
                     if (nb != st) stb[site] = (uint8_t)nb;
                     if (!em) continue;
                     const int dir = detect_decide_from(P, sb, site, step, sid, em);
-                    if (dir >= 0) cd_winner(sh, site, dir, err);
+                    if (dir >= 0) cd_winner(sh, site, dir, err, sp, b);
                 }
             }
         }
@@ -528,7 +538,8 @@ __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int 
 
 // grid = batch * cs CTAs in clusters of cs; phases: bit 0 S2, bit 1 S3 (detect + apply)
 __global__ void __launch_bounds__(CD_THREADS, 4) k_cells_divide(KParams P, Lattice L, int cur, const long long *__restrict__ d_step, int k,
-                                                                const uint32_t *__restrict__ occ, int cs, int phases, int *__restrict__ err, int b0, int *__restrict__ lys)
+                                                                const uint32_t *__restrict__ occ, int cs, int phases, int *__restrict__ err, int b0, int *__restrict__ lys,
+                                                                const SpillArgs sp)
 {
     __shared__ CDShared sh;
     const int b = b0 + blockIdx.x / cs, rank = blockIdx.x % cs;
@@ -536,7 +547,8 @@ __global__ void __launch_bounds__(CD_THREADS, 4) k_cells_divide(KParams P, Latti
     const uint32_t nblk = (uint32_t)(P.n >> 8);
     const uint32_t *occ_b = occ + (size_t)b * nblk;
     if (threadIdx.x == 0) { sh.nwin = 0; sh.nP = (phases & 1) ? 0u : (uint32_t)CD_PCAP + 1u; }
-    if (phases & 1) cd_pass<0>(P, L, cur, b, rank, cs, step, occ_b, nblk, sh, err, lys + b, false);
+    if (rank == 0 && threadIdx.x == 0 && (phases & 2)) sp.n[b] = 0;             // ordered before the first winner by the barrier below
+    if (phases & 1) cd_pass<0>(P, L, cur, b, rank, cs, step, occ_b, nblk, sh, err, lys + b, false, sp);
     if (phases & 2) {
         if (cs > 1) cluster_sync_all(); else __syncthreads();                 // every S2 write of this simulation is visible
         // A READY parent found without an EMPTY neighbour stays blocked until a site of its simulation is vacated, and
@@ -554,14 +566,22 @@ __global__ void __launch_bounds__(CD_THREADS, 4) k_cells_divide(KParams P, Latti
                 if ((em == 0u) != (was != 0u)) L.state[sbase + site] = (uint8_t)(em ? (__ldcg(sb + site) & ~CA_BLOCKED) : (__ldcg(sb + site) | CA_BLOCKED));
                 if (!em) continue;
                 const int dir = detect_decide_from(P, sb, site, step, P.sim_id_base + (uint32_t)b, em);
-                if (dir >= 0) cd_winner(sh, site, dir, err);
+                if (dir >= 0) cd_winner(sh, site, dir, err, sp, b);
             }
         } else {
-            cd_pass<1>(P, L, cur, b, rank, cs, step, occ_b, nblk, sh, err, lys + b, trust);
+            cd_pass<1>(P, L, cur, b, rank, cs, step, occ_b, nblk, sh, err, lys + b, trust, sp);
         }
         if (cs > 1) cluster_sync_all(); else __syncthreads();                 // every decision is taken: now write
         const uint32_t nw = min(sh.nwin, (uint32_t)CD_WINCAP);
         for (uint32_t w = threadIdx.x; w < nw; w += CD_THREADS) apply_winner(P, L, b, sh.win[w] >> 3, (int)(sh.win[w] & 7u), step);
+        if (sh.nwin > (uint32_t)CD_WINCAP || cs > 1) {                            // spilled winners of this simulation: shared out over the cluster
+            const uint32_t ns = min(*(volatile unsigned int *)(sp.n + b), sp.cap_per_sim);
+            const unsigned long long *sl = sp.list + (size_t)b * sp.cap_per_sim;
+            for (uint32_t w = (uint32_t)rank * CD_THREADS + threadIdx.x; w < ns; w += (uint32_t)cs * CD_THREADS) {
+                const unsigned long long ent = __ldcg(sl + w);
+                apply_winner(P, L, b, (uint32_t)(ent >> 3), (int)(ent & 7ull), step);
+            }
+        }
         if (rank == 0 && threadIdx.x == 0) lys[b] = 0;                        // every CTA of the cluster read it before the second barrier
     }
 }

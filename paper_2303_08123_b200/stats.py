@@ -59,3 +59,63 @@ def same_distribution(a, b, alpha=0.01):
     _, _, pt = welch_t(a, b)
     _, pk = ks_2samp(a, b)
     return (pt is None or pt >= alpha) and pk >= alpha
+
+
+def normal_cdf(x):
+    return 0.5 * (1.0 + np.vectorize(math.erf)(np.asarray(x, np.float64) / math.sqrt(2.0)))
+
+
+def ks_normality(a):
+    """One-sample Kolmogorov-Smirnov test of `a` against the normal distribution with the sample's own mean and sd
+    (PAPER.md l.69 and Fig. 3C/D, l.357: "KS-test for the normality of the GPU evaluations"; l.252: the final count over
+    seeds is close to normal).  Returns (D, asymptotic p).  The parameters are estimated from the sample, as in the
+    paper's figure, so p is conservative (Lilliefors); it is used as a sanity threshold, not as an exact level."""
+    a = np.sort(np.asarray(a, np.float64))
+    n = len(a)
+    sd = a.std(ddof=1)
+    if sd == 0.0:
+        return 1.0, 0.0
+    cdf = normal_cdf((a - a.mean()) / sd)
+    d = float(max((np.arange(1, n + 1) / n - cdf).max(), (cdf - np.arange(0, n) / n).max()))
+    en = math.sqrt(n)
+    lam = (en + 0.12 + 0.11 / en) * d
+    p = 2.0 * sum((-1) ** (k - 1) * math.exp(-2.0 * (k * lam) ** 2) for k in range(1, 101))
+    return d, float(min(1.0, max(0.0, p)))
+
+
+def mean_ci95(a):
+    """mean and half-width of its 95 % confidence interval over replicates (Fig. 3A)"""
+    a = np.asarray(a, np.float64)
+    n = len(a)
+    if n < 2:
+        return float(a.mean()), float("inf")
+    try:
+        from scipy import stats as st
+        tq = float(st.t.ppf(0.975, n - 1))
+    except ImportError:
+        tq = 1.96 + 2.4 / max(1, n - 1)
+    return float(a.mean()), tq * float(a.std(ddof=1)) / math.sqrt(n)
+
+
+def compare_implementations(x, y):
+    """The paper's fidelity check between two implementations (Fig. 3A-B): `x`, `y` are
+    [protocols][replicates] final counts (or fitness).  Per protocol: mean and 95 % half-width of each, two-sided
+    Welch t-test p-value, two-sample KS p-value.  Returns a dict of arrays."""
+    x, y = [np.asarray(r, np.float64) for r in x], [np.asarray(r, np.float64) for r in y]
+    assert len(x) == len(y)
+    out = {k: [] for k in ("mean_x", "ci_x", "mean_y", "ci_y", "p_t", "p_ks")}
+    for a, b in zip(x, y):
+        ma, ca = mean_ci95(a)
+        mb, cb = mean_ci95(b)
+        out["mean_x"].append(ma); out["ci_x"].append(ca); out["mean_y"].append(mb); out["ci_y"].append(cb)
+        out["p_t"].append(welch_t(a, b)[2]); out["p_ks"].append(ks_2samp(a, b)[1])
+    return {k: np.array(v, np.float64) for k, v in out.items()}
+
+
+def pvalues_not_piled_up(p, level=0.05, slack=3.0):
+    """Under the null hypothesis p-values are uniform: about `level` of them fall below `level`.  True unless the
+    fraction below `level` exceeds `level` by more than `slack` binomial standard deviations (and at least 2 do)."""
+    p = np.asarray(p, np.float64)
+    n = len(p)
+    k = int((p < level).sum())
+    return k <= max(1.0, n * level + slack * math.sqrt(n * level * (1.0 - level)))

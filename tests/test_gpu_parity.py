@@ -220,7 +220,7 @@ def test_state_roundtrip_broadcast_and_errors():
     ((32, 32, 12), 4, {}),                                   # fixed 32x32 kernel, map from the diffusion kernel, default cluster
     ((64, 64, 10), 4, {"cluster": 1}),                       # fixed 64x64 kernel
     ((64, 64, 10), 4, {"cluster": 2, "graph_steps": 4}),     # clustered S2+S3 across 2 CTAs, inside CUDA graphs
-    ((64, 64, 10), 4, {"chains": 2, "graph_steps": 4}),      # two half-batch chains on forked streams
+    ((64, 64, 10), 4, {"graph_steps": 4}),                   # short CUDA graphs
     ((64, 64, 10), 4, {"cell_path": 0}),                     # generic scan kernels next to the fused diffusion
     ((32, 32, 12), 3, {}),                                   # 3 fused levels
     ((32, 32, 12), 6, {"graph_steps": 4}),                   # 3 + 3 levels, two passes (buffer flips twice per step)
