@@ -225,6 +225,7 @@ int enqueue_advance(ca_ctx *c, int adv)
 int run_plain(ca_ctx *c, long long nsteps)
 {
     const int G = c->graph_steps;
+    if (c->launch_err != cudaSuccess) { const cudaError_t le = c->launch_err; c->launch_err = cudaSuccess; return cuda_fail(c, le, "kernel launch"); }
     while (G > 0 && nsteps >= G) {
         const int par = c->cur;
         if (!c->graph[par] || c->graph_len[par] != G) {

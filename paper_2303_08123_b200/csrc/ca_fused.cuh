@@ -37,6 +37,7 @@ constexpr int F_PY = 4;        // rows per lane
 constexpr int F_RING = 3;      // field-plane ring depth = register phase count (prefetch distance 2)
 constexpr int F_SRING = 8;     // state-plane ring depth (a plane is used by NL consecutive iterations)
 constexpr int F_MAXNL = 4;
+constexpr int F_MAXSLAB = 8;
 constexpr int F_MAXGRID = 640; // persistent CTAs at most (the split table travels as a kernel parameter)
 
 struct FusedArgs {
@@ -49,10 +50,11 @@ struct FusedArgs {
     int always_slow[3];        // 1: the clamp cannot be proven idle for this lambda -> always take the full path
     float zero;                // 0.0f, opaque to ptxas (see Fused::level)
     uint32_t *occ;             // occupancy map for S2/S3 (one bit per 8 state bytes), written by the fixed-size kernels; may be NULL
-    // tiled variant (nx or ny > 64): the plane is cut into ntx * nty tiles of at most 64 x 64 sites including a halo of
-    // F_MAXNL sites towards neighbouring tiles; tile t loads [t0, t1) and stores its output window [o0, o1)
-    int ntx, nty;
-    short tx0[4], tx1[4], ox0[4], ox1[4], ty0[4], ty1[4], oy0[4], oy1[4];
+    // slab variant (planes wider or taller than 64 sites): a plane is cut along y into nslab slabs of whole rows; slab s
+    // loads rows [sy0, sy1) -- its output rows [so0, so1) plus a halo of F_MAXNL rows towards neighbouring slabs -- and a
+    // row is covered by nxb column blocks of 2*LRP sites (rga = row groups of F_PY rows a CTA holds)
+    int nslab, nxb, rga;
+    short sy0[F_MAXSLAB], sy1[F_MAXSLAB], so0[F_MAXSLAB], so1[F_MAXSLAB];
 };
 
 // ---- packed f32x2 arithmetic (Blackwell FADD2/FMUL2/FFMA2); .rn, no ftz: identical to two scalar ops ----
@@ -91,10 +93,20 @@ __device__ __forceinline__ u64 lds64(uint32_t a) { u64 v; asm volatile("ld.share
 __device__ __forceinline__ void sts64(uint32_t a, u64 v) { asm volatile("st.shared.b64 [%0], %1;" ::"r"(a), "l"(v) : "memory"); }
 __device__ __forceinline__ uint32_t lds16(uint32_t a) { uint32_t v; asm volatile("ld.shared.u16 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
 __device__ __forceinline__ float lds32f(uint32_t a) { float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a)); return v; }
+__device__ __forceinline__ float4 lds128f(uint32_t a)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ void sts128f(uint32_t a, float x, float y, float z, float w)
+{
+    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(a), "f"(x), "f"(y), "f"(z), "f"(w) : "memory");
+}
 
 struct FusedGeom {             // host-computed launch geometry, passed by value
     int nwarps, ngroups_alloc; // strips of F_PY rows: groups = nwarps * (32 / LRP)
-    uint32_t off_lut, off_in, off_st, off_ex, smem_bytes;
+    uint32_t off_lut, off_in, off_st, off_ex, off_xex, smem_bytes;
     long long total_planes;    // batch * 3 * (nz - 2): the flattened (unit, interior plane) space
     int start[F_MAXGRID + 1];  // CTA g works on flattened planes [start[g], start[g+1]) (cost-balanced on the host)
 };
@@ -104,7 +116,6 @@ struct FusedCtx {
     const float *src;          // field of this unit, already offset to this lane's (x0, y0)
     float *dst;
     const float *src_plane0;   // unit base (for the bulk copies)
-    const uint8_t *st_src;     // tiled variant: state of this unit at this lane's (x0, y0)
     const uint8_t *st_plane0;
     int nx, nxny, nz;          // run-time geometry (ignored by the fixed-size instantiations)
     uint32_t ex_lvl;
@@ -123,42 +134,62 @@ struct FusedCtx {
     uint32_t rowmask;          // bit j: row y0+j exists and this lane's x pair is inside the lattice
     bool strip_ok;
     uint32_t *occ_row;         // species 0 only: occupancy words of this warp's strip, indexed by plane (else NULL)
+    // slab variant
+    uint32_t in_slot, st_slot;     // bytes of one ring slot (the tallest slab)
+    uint32_t ld_fbytes, ld_sbytes; // bytes of this slab's rows of a field / state plane
+    uint32_t yst;                  // bytes of one row of the y-exchange (a whole lattice row)
+    uint32_t xs_w, xs_r, xel;      // x-seam exchange between column blocks: my store / load slot (buffer 0, level 0), bytes per level
+    bool seam, seam_r;             // this lane sits on a seam between two column blocks; ... on the right edge of its block
+    uint32_t occ_w0, occ_nw;       // species 0: occupancy words of a plane this slab is responsible for
+    uint32_t occ_soff;             // byte offset of word occ_w0 inside the state slot (may wrap negative never: halo covers it)
 };
 
 // NX = NY = 0: lattice dims at run time (any even nx <= 2*LRP); otherwise compile-time dims, all address math folds
-template <int NL, int LRP, int NX, int NY, bool TILED = false>
+// SLAB: planes larger than a CTA holds; NX, NY then give the lattice (NX = nxb * 2 * LRP) and the CTA works on y-slabs
+template <int NL, int LRP, int NX, int NY, bool SLAB = false>
 struct Fused {
     static constexpr bool FIXED = NX != 0;
     static constexpr int RW = 32 / LRP;
-    // every lane and row holds valid data: whole fixed-size planes, or a tile (lanes / strips outside a tile are clamped onto
-    // its last columns / rows: they compute duplicates that feed only the frozen outer ring and are never stored)
-    static constexpr bool FULL = TILED || (FIXED && NX == 2 * LRP && NY % (F_PY * RW) == 0);
-    static constexpr uint32_t GRP = LRP * 8u;                                         // bytes of one exchanged row
-    static constexpr uint32_t EXL = TILED ? 2u * (16u + 2u) * GRP                     // tiles: 16 strips allocated
-                                          : (FIXED ? 2u * (((NY + F_PY * RW - 1) / (F_PY * RW)) * RW + 2u) * GRP : 0u);
+    static constexpr int NXB = (SLAB && FIXED) ? NX / (2 * LRP) : 1;                 // column blocks (slab variant with compile-time dims)
+    static constexpr int RGA = (SLAB && FIXED) ? (16 * RW) / NXB : 0;                // row groups a CTA of 16 warps holds
+    // every lane and row holds valid data: whole fixed-size planes, or a slab (groups beyond a short slab are clamped onto its
+    // last row group: they compute duplicates that feed only the frozen last row and are never stored)
+    static constexpr bool FULL = SLAB || (FIXED && NX == 2 * LRP && NY % (F_PY * RW) == 0);
+    static constexpr uint32_t GRP = LRP * 8u;                                         // bytes one row group exchanges per row
+    static constexpr uint32_t EXL = SLAB ? 2u * (uint32_t)(RGA + 2) * (uint32_t)NX * 4u
+                                         : (FIXED ? 2u * (((NY + F_PY * RW - 1) / (F_PY * RW)) * RW + 2u) * GRP : 0u);
+    static constexpr uint32_t XEL = (uint32_t)(RGA * NXB) * 32u;                      // x-seam exchange, bytes per level
 
     static __device__ __forceinline__ int nx(const FusedCtx &c) { return FIXED ? NX : c.nx; }
     static __device__ __forceinline__ int nxny(const FusedCtx &c) { return FIXED ? NX * NY : c.nxny; }
-    static __device__ __forceinline__ uint32_t exl(const FusedCtx &c) { return (FIXED || TILED) ? EXL : c.ex_lvl; }
+    static __device__ __forceinline__ uint32_t exl(const FusedCtx &c) { return FIXED ? EXL : c.ex_lvl; }
+    static __device__ __forceinline__ uint32_t xel(const FusedCtx &c) { return FIXED ? XEL : c.xel; }
+    static __device__ __forceinline__ uint32_t yst(const FusedCtx &c) { return SLAB ? (FIXED ? (uint32_t)NX * 4u : c.yst) : GRP; }
     static __device__ __forceinline__ bool row(const FusedCtx &c, int j) { return FULL ? true : ((c.rowmask >> j) & 1u) != 0u; }
-    // tiled variant: the rings hold a tile with a fixed pitch of 64 sites; only the tile's output window is stored
-    static __device__ __forceinline__ bool srow(const FusedCtx &c, int j) { return TILED ? ((c.rowmask >> (16 + j)) & 1u) != 0u : row(c, j); }
-    static __device__ __forceinline__ uint32_t stpitch(const FusedCtx &c) { return TILED ? 64u : (uint32_t)nx(c); }
-    static __device__ __forceinline__ uint32_t stslot(const FusedCtx &c) { return TILED ? 64u * 64u : (uint32_t)nxny(c); }
-    static __device__ __forceinline__ uint32_t inpitch(const FusedCtx &c) { return TILED ? 256u : (uint32_t)nx(c) * 4u; }
-    static __device__ __forceinline__ uint32_t inslot(const FusedCtx &c) { return TILED ? 64u * 256u : (uint32_t)nxny(c) * 4u; }
+    // slab variant: only the slab's output rows are stored (and only by the groups that are not clamped duplicates)
+    static __device__ __forceinline__ bool srow(const FusedCtx &c, int j) { return SLAB ? ((c.rowmask >> (16 + j)) & 1u) != 0u : row(c, j); }
+    static __device__ __forceinline__ uint32_t stpitch(const FusedCtx &c) { return (uint32_t)nx(c); }
+    static __device__ __forceinline__ uint32_t stslot(const FusedCtx &c) { return SLAB ? ((FIXED) ? (uint32_t)(RGA * F_PY * NX) : c.st_slot) : (uint32_t)nxny(c); }
+    static __device__ __forceinline__ uint32_t inpitch(const FusedCtx &c) { return (uint32_t)nx(c) * 4u; }
+    static __device__ __forceinline__ uint32_t inslot(const FusedCtx &c) { return SLAB ? ((FIXED) ? (uint32_t)(RGA * F_PY * NX) * 4u : c.in_slot) : (uint32_t)nxny(c) * 4u; }
 
     // the diffusion part of one sub-step of [D S1] for this lane's 2 x 4 points; C = centre plane, M/P = planes z-1/z+1
     static __device__ __forceinline__ void level(const u64 (&M)[F_PY], const u64 (&C)[F_PY], const u64 (&P)[F_PY], u64 (&N)[F_PY],
-                                                 u64 up, u64 dn, const u64 (&lam2)[F_PY], const u64 zero2)
+                                                 u64 up, u64 dn, const u64 (&lam2)[F_PY], const u64 zero2,
+                                                 const float4 xe, const bool seam_l, const bool seam_r)
     {
         const u64 six2 = pk(6.0f, 6.0f);
+        const float xev[F_PY] = { xe.x, xe.y, xe.z, xe.w };
 #pragma unroll
         for (int j = 0; j < F_PY; ++j) {
             float c0, c1;
             upk(C[j], c0, c1);
-            const float xl = __shfl_up_sync(0xFFFFFFFFu, c1, 1, LRP);      // value at x0-1 (own c1 at the strip edge: WALL side, unused)
-            const float xr = __shfl_down_sync(0xFFFFFFFFu, c0, 1, LRP);    // value at x0+2
+            float xl = __shfl_up_sync(0xFFFFFFFFu, c1, 1, LRP);            // value at x0-1 (own c1 at the strip edge: WALL side, unused)
+            float xr = __shfl_down_sync(0xFFFFFFFFu, c0, 1, LRP);          // value at x0+2
+            if constexpr (SLAB) {                                           // seam between two column blocks: the neighbour block's edge column
+                xl = seam_l ? xev[j] : xl;
+                xr = seam_r ? xev[j] : xr;
+            }
             const u64 xs = pk(__fadd_rn(xl, c1), __fadd_rn(c0, xr));       // xm + xp
             const u64 ys = add2(j == 0 ? up : C[j > 0 ? j - 1 : 0], j == F_PY - 1 ? dn : C[j < F_PY - 1 ? j + 1 : 0]);   // ym + yp
             const u64 zs = add2(M[j], P[j]);                                 // zm + zp
@@ -170,25 +201,19 @@ struct Fused {
         }
     }
 
-    // tiled variant: every lane copies its own 4 x 8 field bytes (and, even lanes, 4 x 4 state bytes) of iteration i with
-    // cp.async; one commit group per iteration, empty when there is nothing to load, so that the group count stays uniform
-    static __device__ __forceinline__ void tile_copy(const FusedCtx &c, int i, int slot)
+    // slab variant: a lane on a seam publishes its edge column (F_PY rows) of level K for the neighbouring column block
+    static __device__ __forceinline__ void seam_store(const FusedCtx &c, const uint32_t addr, const u64 (&V)[F_PY])
     {
-        const int t = c.t0 + i;
-        if (i < c.nsteps && t >= c.ld_lo && t < c.ld_hi) {
-            const float *g = c.src + (size_t)t * nxny(c);
-            const uint8_t *gs = c.st_src + (size_t)t * nxny(c);
-            const uint32_t d = c.in_lane + (uint32_t)slot * inslot(c);
-            const uint32_t ds = c.st_lane + ((c.itg + (uint32_t)i) & (F_SRING - 1)) * stslot(c);
+        if (c.seam) {
+            float e[F_PY];
 #pragma unroll
-            for (int j = 0; j < F_PY; ++j)
-                if (row(c, j)) {
-                    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d + (uint32_t)j * 256u), "l"(g + j * nx(c)) : "memory");
-                    if (!(threadIdx.x & 1))
-                        asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(ds + (uint32_t)j * 64u), "l"(gs + j * nx(c)) : "memory");
-                }
+            for (int j = 0; j < F_PY; ++j) {
+                float a, b;
+                upk(V[j], a, b);
+                e[j] = c.seam_r ? b : a;
+            }
+            sts128f(addr, e[0], e[1], e[2], e[3]);
         }
-        asm volatile("cp.async.commit_group;" ::: "memory");
     }
 
     // producer (one thread): start the bulk copies of iteration i into field-ring slot i mod 3
@@ -196,11 +221,11 @@ struct Fused {
     {
         const int t = c.t0 + i;
         const uint32_t bar = c.bars + 8u * (uint32_t)slot;
-        const uint32_t pb = (uint32_t)nxny(c) * 4u, sb = (uint32_t)nxny(c);
+        const uint32_t pb = SLAB ? c.ld_fbytes : (uint32_t)nxny(c) * 4u, sb = SLAB ? c.ld_sbytes : (uint32_t)nxny(c);   // a slab's rows are contiguous
         if (t >= c.ld_lo && t < c.ld_hi) {
             mbar_expect_tx(bar, pb + sb);
-            bulk_g2s(c.in_ring + (uint32_t)slot * pb, c.src_plane0 + (size_t)t * nxny(c), pb, bar);
-            bulk_g2s(c.st_ring + ((c.itg + (uint32_t)i) & (F_SRING - 1)) * sb, c.st_plane0 + (size_t)t * nxny(c), sb, bar);
+            bulk_g2s(c.in_ring + (uint32_t)slot * inslot(c), c.src_plane0 + (size_t)t * nxny(c), pb, bar);
+            bulk_g2s(c.st_ring + ((c.itg + (uint32_t)i) & (F_SRING - 1)) * stslot(c), c.st_plane0 + (size_t)t * nxny(c), sb, bar);
         } else {
             mbar_arrive(bar);
         }
@@ -209,7 +234,7 @@ struct Fused {
     // level K (sub-step K) at iteration i: computes plane t-K; outside the steady range it may idle or copy a WALL plane
     template <int PH, int K, bool STEADY, bool NOCELLS>
     static __device__ __forceinline__ void levels(const int t, const uint32_t q, const uint32_t exr, const uint32_t exw,
-                                                  u64 (&h)[NL][3][F_PY], FusedCtx &c)
+                                                  const uint32_t xsr, const uint32_t xsw, u64 (&h)[NL][3][F_PY], FusedCtx &c)
     {
         if constexpr (K <= NL) {
             constexpr int sm = (PH - K - 1 + 12) % 3, sc = (PH - K + 12) % 3, sp = (PH - K + 1 + 12) % 3;
@@ -219,11 +244,15 @@ struct Fused {
             if (!STEADY) compute = zc >= max(1, c.za - (NL - K)) && zc < min(c.nz - 1, c.zb + (NL - K));
             if (compute) {
                 const uint32_t el = exl(c);
-                const u64 up = lds64(exr + (uint32_t)(K - 1) * el + (el / 2 - GRP));     // bottom row of the strip above
-                const u64 dn = lds64(exr + (uint32_t)(K - 1) * el + GRP);                // top row of the strip below
+                const u64 up = lds64(exr + (uint32_t)(K - 1) * el + (el / 2 - yst(c)));  // bottom row of the strip above
+                const u64 dn = lds64(exr + (uint32_t)(K - 1) * el + yst(c));             // top row of the strip below
+                float4 xe = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                if constexpr (SLAB) {
+                    if (c.seam) xe = lds128f(xsr + (uint32_t)(K - 1) * xel(c));                  // the neighbour block's edge column, written by the previous iteration
+                }
                 u64 nloc[F_PY];
                 u64 (&N)[F_PY] = *(K < NL ? &h[KO][sc] : &nloc);
-                level(h[K - 1][sm], h[K - 1][sc], h[K - 1][sp], N, up, dn, c.lam2, c.zero2);
+                level(h[K - 1][sm], h[K - 1][sc], h[K - 1][sp], N, up, dn, c.lam2, c.zero2, xe, c.seam && !c.seam_r, c.seam_r);
                 if (!NOCELLS && (((c.flags | c.slowmask) >> K) & 1u)) {    // cells in this strip: source term and clamp
                     const uint32_t s = c.st_lane + ((q - (uint32_t)K) & (F_SRING - 1)) * stslot(c);
 #pragma unroll
@@ -238,6 +267,7 @@ struct Fused {
                 if constexpr (K < NL) {
                     sts64(exw + (uint32_t)K * el, N[0]);
                     sts64(exw + (uint32_t)K * el + el / 2, N[F_PY - 1]);
+                    if constexpr (SLAB) seam_store(c, xsw + (uint32_t)K * xel(c), N);
                 } else {
                     float *o = c.dst + (size_t)zc * nxny(c);
 #pragma unroll
@@ -258,7 +288,7 @@ struct Fused {
                     h[KO][sc][j] = pk(v.x, v.y);
                 }
             }
-            levels<PH, K + 1, STEADY, NOCELLS>(t, q, exr, exw, h, c);
+            levels<PH, K + 1, STEADY, NOCELLS>(t, q, exr, exw, xsr, xsw, h, c);
         }
     }
 
@@ -278,20 +308,19 @@ struct Fused {
     {
         const int t = c.t0 + i;
         const uint32_t q = c.itg + (uint32_t)i;
-        if constexpr (!TILED) {
-            if (threadIdx.x == 0 && i + (F_RING - 1) < c.nsteps) issue(c, i + (F_RING - 1), (PH + F_RING - 1) % 3);
-        }
+        if (threadIdx.x == 0 && i + (F_RING - 1) < c.nsteps) issue(c, i + (F_RING - 1), (PH + F_RING - 1) % 3);
         const uint32_t exb = exl(c) * NL;                                   // bytes of one exchange buffer
         const uint32_t exw = c.ex_self + ((uint32_t)i & 1u) * exb;          // rows written now, read by the next iteration
         const uint32_t exr = c.ex_self + exb - ((uint32_t)i & 1u) * exb;    // rows written by the previous iteration
-        // ---- level 0: plane t from the ring
-        if constexpr (TILED) {
-            asm volatile("cp.async.wait_group 1;" ::: "memory");             // this iteration's copies have landed (the next one's may be in flight)
-            __syncwarp();                                                   // state bytes are copied by the even lane of each lane pair
-        } else {
-            mbar_wait(c.bars + 8u * PH, (c.par >> PH) & 1u);
-            c.par ^= 1u << PH;
+        uint32_t xsw = 0, xsr = 0;
+        if constexpr (SLAB) {
+            const uint32_t xb = xel(c) * NL;
+            xsw = c.xs_w + ((uint32_t)i & 1u) * xb;
+            xsr = c.xs_r + xb - ((uint32_t)i & 1u) * xb;
         }
+        // ---- level 0: plane t from the ring
+        mbar_wait(c.bars + 8u * PH, (c.par >> PH) & 1u);
+        c.par ^= 1u << PH;
         bool any = false;
         if (STEADY || (t >= c.ld_lo && t < c.ld_hi)) {
             const uint32_t a = c.in_lane + (uint32_t)PH * inslot(c);
@@ -299,27 +328,36 @@ struct Fused {
             for (int j = 0; j < F_PY; ++j) h[0][PH][j] = row(c, j) ? lds64(a + (uint32_t)j * inpitch(c)) : 0ull;
             sts64(exw, h[0][PH][0]);
             sts64(exw + exl(c) / 2, h[0][PH][F_PY - 1]);
+            if constexpr (SLAB) seam_store(c, xsw, h[0][PH]);
             // "cells in my strip": every lane looks at 8 bytes of the warp's strip of the state plane; a byte counts when kind is 1..6
-            if constexpr (TILED) {                                           // tiles are not contiguous: every lane looks at its own 2 x 4 bytes
+            if constexpr (SLAB) {                                            // a warp's points are not contiguous bytes: every lane looks at its own 2 x 4 bytes
                 const uint32_t sa = c.st_lane + (q & (F_SRING - 1)) * stslot(c);
                 uint32_t m = 0;
 #pragma unroll
-                for (int j = 0; j < F_PY; ++j) m |= row(c, j) ? (((lds16(sa + (uint32_t)j * 64u) & 0x0707u) + 0x0101u) & 0x0606u) : 0u;
+                for (int j = 0; j < F_PY; ++j) m |= ((lds16(sa + (uint32_t)j * stpitch(c)) & 0x0707u) + 0x0101u) & 0x0606u;
                 any = m != 0u;
+                // the S2/S3 occupancy map (one bit per 8 consecutive state bytes, one word per 256): this slab's words of the plane,
+                // read from the state slab in shared memory, one word per warp and trip
+                if (c.occ_row != nullptr) {
+                    for (uint32_t w = threadIdx.x >> 5; w < c.occ_nw; w += blockDim.x >> 5) {
+                        const u64 v = lds64(c.st_ring + (q & (F_SRING - 1)) * stslot(c) + c.occ_soff + w * 256u + 8u * (threadIdx.x & 31u));
+                        const uint32_t bal = __ballot_sync(0xFFFFFFFFu, (((v & 0x0707070707070707ull) + 0x0101010101010101ull) & 0x0606060606060606ull) != 0ull);
+                        if ((threadIdx.x & 31) == 0) c.occ_row[(size_t)t * (size_t)(nxny(c) / 256) + c.occ_w0 + w] = bal;
+                    }
+                }
             } else {
                 const u64 w = c.strip_ok ? lds64(c.st_strip + (q & (F_SRING - 1)) * (uint32_t)nxny(c)) : 0ull;
                 any = (((w & 0x0707070707070707ull) + 0x0101010101010101ull) & 0x0606060606060606ull) != 0ull;
             }
         }
-        if constexpr (TILED) tile_copy(c, i + (F_RING - 1), (PH + F_RING - 1) % 3);   // ring slot of iteration i-1: read one iteration ago
         const uint32_t ballot = __ballot_sync(0xFFFFFFFFu, any);
         c.flags = (c.flags << 1) | (ballot ? 1u : 0u);
-        if constexpr (FIXED && !TILED) {                                    // the same vote is the S2/S3 occupancy map: strip = 256 contiguous bytes
+        if constexpr (FIXED && !SLAB) {                                     // the same vote is the S2/S3 occupancy map: strip = 256 contiguous bytes
             if ((threadIdx.x & 31) == 0 && c.occ_row != nullptr && (STEADY || (t >= c.ld_lo && t < c.ld_hi)))
                 c.occ_row[(size_t)t * (NX * NY / 256)] = ballot;
         }
         // ---- levels 1..NL: level k computes plane t-k from level k-1
-        levels<PH, 1, STEADY, NOCELLS>(t, q, exr, exw, h, c);
+        levels<PH, 1, STEADY, NOCELLS>(t, q, exr, exw, xsr, xsw, h, c);
         __syncthreads();
     }
 };
@@ -417,36 +455,54 @@ __global__ void __launch_bounds__(512, 1) k_diffuse_fused(const FusedArgs A, con
     }
 }
 
-// Tiled variant for planes wider than 64 sites (BASELINE configs[2], [3]: 96^3, 80^3).  Same march, same levels; a
-// work unit is (simulation, species, xy-tile, z-range).  A tile carries a halo of F_MAXNL sites towards its neighbour
-// tiles: its outermost ring is frozen (lambda = 0), the garbage that creates moves inwards one site per sub-step and
-// never reaches the output window.  Tiles are not contiguous in memory, so planes arrive by per-lane cp.async
-// (every lane copies exactly the sites it owns: no barrier needed for the field ring).
-// NXG, NYG: lattice dims at compile time (row pitch and plane size fold into the copy / store addresses); 0 = run time
-template <int NL, int NXG, int NYG>
-__global__ void __launch_bounds__(512, 1) k_diffuse_tiled(const FusedArgs A, const FusedGeom Gm)
+// Slab variant for planes a CTA cannot hold whole (BASELINE configs[2], [3]: 96^3, 80^3).  Same march, same levels, same
+// bulk-copy rings; a work unit is (simulation, species, y-slab, z-range).  A slab is a range of WHOLE rows of the plane --
+// contiguous in memory, so it arrives by the same 1-D bulk copies as a whole plane -- and carries a halo of F_MAXNL rows
+// towards its neighbour slabs: its first / last row is frozen (lambda = 0; on the lattice face that is the WALL), the error
+// that creates at a cut moves inwards one row per sub-step and never reaches the output rows.  A row is wider than one
+// row group of LRP lanes, so it is covered by nxb column blocks side by side; x-neighbours across a seam between two blocks
+// go through a small shared-memory exchange (one 16-byte store and load per lane on a seam and level), exactly like the
+// y-neighbours across row groups.  The S2/S3 occupancy map is written from the state slab while it is in shared memory.
+// NXG, NYG: lattice dims at compile time (all strides fold); 0 = run time.
+template <int NL, int LRP, int NXG, int NYG>
+__global__ void __launch_bounds__(512, 1) k_diffuse_slab(const FusedArgs A, const FusedGeom Gm)
 {
-    typedef Fused<NL, 32, NXG, NYG, true> F;
+    typedef Fused<NL, LRP, NXG, NYG, true> F;
     extern __shared__ __align__(128) unsigned char fsm[];
+    constexpr int RW = 32 / LRP;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int lx = lane, g = warp;
+    const int lx = lane % LRP, gi = warp * RW + lane / LRP;
+    const int nxb = NXG ? NXG / (2 * LRP) : A.nxb, rga = NXG ? (16 * RW) / (NXG / (2 * LRP)) : A.rga;
+    const int blk = gi % nxb, rg = gi / nxb;                                  // column block, row group inside the slab
+    const int nxr = NXG ? NXG : A.nx, nyr = NYG ? NYG : A.ny;
+    const int x0 = blk * 2 * LRP + 2 * lx;
     const uint32_t base = smem_u32(fsm);
 
     FusedCtx c;
-    c.nx = A.nx; c.nxny = A.nx * A.ny; c.nz = A.nz;
+    c.nx = nxr; c.nxny = nxr * nyr; c.nz = A.nz;
     c.bars = base; c.in_ring = base + Gm.off_in; c.st_ring = base + Gm.off_st;
-    c.in_lane = c.in_ring + (uint32_t)(F_PY * g) * 256u + (uint32_t)lx * 8u;
-    c.st_lane = c.st_ring + (uint32_t)(F_PY * g) * 64u + (uint32_t)lx * 2u;
-    c.st_strip = 0; c.strip_ok = false; c.occ_row = nullptr; c.src_plane0 = nullptr; c.st_plane0 = nullptr;
-    c.ex_lvl = 2u * (uint32_t)(Gm.ngroups_alloc + 2) * F::GRP;
-    c.ex_self = base + Gm.off_ex + (uint32_t)(g + 1) * F::GRP + (uint32_t)lx * 8u;
+    c.in_slot = (uint32_t)(rga * F_PY * nxr) * 4u; c.st_slot = (uint32_t)(rga * F_PY * nxr);
+    c.yst = (uint32_t)nxr * 4u;
+    c.ex_lvl = 2u * (uint32_t)(rga + 2) * c.yst;                               // [top rows | bottom rows] of rga + 2 lattice rows (a zero row at both ends)
+    c.ex_self = base + Gm.off_ex + (uint32_t)(rg + 1) * c.yst + (uint32_t)x0 * 4u;
+    c.xel = (uint32_t)(rga * nxb) * 32u;                                       // per level: [row group][block][left edge | right edge] x 16 bytes
+    c.seam_r = lx == LRP - 1 && blk < nxb - 1;
+    c.seam = c.seam_r || (lx == 0 && blk > 0);
+    c.xs_w = base + Gm.off_xex + (uint32_t)((rg * nxb + blk) * 2 + (c.seam_r ? 1 : 0)) * 16u;
+    c.xs_r = base + Gm.off_xex + (uint32_t)((rg * nxb + blk + (c.seam_r ? 1 : -1)) * 2 + (c.seam_r ? 0 : 1)) * 16u;   // the neighbour block's facing edge
+    c.st_strip = 0; c.strip_ok = false;
     c.itg = 0; c.par = 0;
     c.zero2 = pk(A.zero, A.zero);
+    if (tid == 0) {
+#pragma unroll
+        for (int r = 0; r < F_RING; ++r) mbar_init(c.bars + 8u * r, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
     for (int e = tid; e < 96; e += blockDim.x) reinterpret_cast<float *>(fsm + Gm.off_lut)[e] = A.lut[e / 32][e % 32];
-    for (uint32_t e = tid; e < 2u * NL * c.ex_lvl / 8u; e += blockDim.x) reinterpret_cast<u64 *>(fsm + Gm.off_ex)[e] = 0ull;
+    for (uint32_t e = tid; e < (Gm.smem_bytes - Gm.off_ex) / 8u; e += blockDim.x) reinterpret_cast<u64 *>(fsm + Gm.off_ex)[e] = 0ull;   // both exchanges
     __syncthreads();
 
-    const int nzi = A.nz - 2, ntiles = A.ntx * A.nty;
+    const int nzi = A.nz - 2;
     long long p = Gm.start[blockIdx.x];
     const long long p_end = Gm.start[blockIdx.x + 1];
     u64 h[NL][3][F_PY];
@@ -459,43 +515,46 @@ __global__ void __launch_bounds__(512, 1) k_diffuse_tiled(const FusedArgs A, con
 
     while (p < p_end) {
         const int unit = (int)(p / nzi);
-        const int tile = unit % ntiles, us = unit / ntiles;
+        const int slab = unit % A.nslab, us = unit / A.nslab;
         const int b = us / 3, sp = us % 3;
-        const int tix = tile % A.ntx, tiy = tile / A.ntx;
         c.za = 1 + (int)(p - (long long)unit * nzi);
         c.zb = (int)min((long long)(A.nz - 1), (long long)c.za + (p_end - p));
         p += c.zb - c.za;
-        const int x = A.tx0[tix] + 2 * lx, y0 = A.ty0[tiy] + F_PY * g;
-        const int xc = min(x, A.tx1[tix] - 2), yc = min(y0, A.ty1[tiy] - F_PY);   // clamped: always inside the tile
+        const int ty0 = A.sy0[slab], ty1 = A.sy1[slab], oy0 = A.so0[slab], oy1 = A.so1[slab];
+        const int y0 = ty0 + F_PY * rg;
+        const int yc = min(y0, ty1 - F_PY);                                    // groups beyond a short slab: duplicates of its last row group
         const size_t ubase = (size_t)b * (size_t)c.nxny * (size_t)A.nz;
-        c.src = A.src[sp] + ubase + (yc * A.nx + xc);
-        c.dst = A.dst[sp] + ubase + (yc * A.nx + xc);                          // stores are masked with the unclamped position
-        c.st_src = A.state + ubase + (yc * A.nx + min(x, A.tx1[tix] - 4));     // even lanes copy 4 state bytes
+        c.src_plane0 = A.src[sp] + ubase + (size_t)ty0 * nxr;
+        c.st_plane0 = A.state + ubase + (size_t)ty0 * nxr;
+        c.ld_fbytes = (uint32_t)((ty1 - ty0) * nxr) * 4u; c.ld_sbytes = (uint32_t)((ty1 - ty0) * nxr);
+        c.src = A.src[sp] + ubase + (yc * nxr + x0);
+        c.dst = A.dst[sp] + ubase + (yc * nxr + x0);
+        c.in_lane = c.in_ring + (uint32_t)((yc - ty0) * nxr + x0) * 4u;
+        c.st_lane = c.st_ring + (uint32_t)((yc - ty0) * nxr + x0);
         c.t0 = c.za - NL;
         c.nsteps = c.zb - c.za + 2 * NL;
         c.ld_lo = max(0, c.za - NL); c.ld_hi = min(A.nz, c.zb + NL);
         c.st_lo = 2 * NL; c.st_hi = min(A.nz, c.zb + NL) - c.t0;
         c.flags = 0; c.slowmask = A.always_slow[sp] ? 0xFFFFFFFFu : 0u;
         c.lut = base + Gm.off_lut + (uint32_t)sp * 128u;
+        // occupancy words of a plane whose first byte lies in this slab's output rows (the halo covers the rest of the word)
+        c.occ_row = (sp == 0 && A.occ != nullptr) ? A.occ + (size_t)b * (size_t)(c.nxny / 256) * (size_t)A.nz : nullptr;
+        c.occ_w0 = (uint32_t)((oy0 * nxr + 255) / 256);
+        c.occ_nw = (uint32_t)((oy1 * nxr + 255) / 256) - c.occ_w0;
+        c.occ_soff = c.occ_w0 * 256u - (uint32_t)(ty0 * nxr);
         const float lam = A.lam[sp];
         c.rowmask = 0;
-        const bool xin = x < A.tx1[tix];
-        const bool xout = x >= A.ox0[tix] && x < A.ox1[tix];
 #pragma unroll
         for (int j = 0; j < F_PY; ++j) {
             const int y = y0 + j;
-            if (xin && y < A.ty1[tiy]) c.rowmask |= 1u << j;
-            if (xout && y >= A.oy0[tiy] && y < A.oy1[tiy]) c.rowmask |= 1u << (16 + j);
-            const bool rowin = y > A.ty0[tiy] && y < A.ty1[tiy] - 1;          // the tile's outer ring is frozen (WALL, or halo edge)
-            c.lam2[j] = pk(rowin && x > A.tx0[tix] && x < A.tx1[tix] - 1 ? lam : 0.0f, rowin && x + 1 < A.tx1[tix] - 1 ? lam : 0.0f);
+            if (y0 == yc && y >= oy0 && y < oy1) c.rowmask |= 1u << (16 + j);
+            const bool rowin = y > ty0 && y < ty1 - 1;                           // the slab's first / last row is frozen (WALL, or halo edge)
+            c.lam2[j] = pk(rowin && x0 > 0 ? lam : 0.0f, rowin && x0 + 1 < nxr - 1 ? lam : 0.0f);
         }
         const int i0 = ((c.ld_lo - c.t0) / 3) * 3;
-        c.t0 += i0; c.nsteps -= i0; c.st_lo = max(0, c.st_lo - i0); c.st_hi -= i0;   // re-base: iteration 0 is the first useful one
-        asm volatile("cp.async.wait_group 0;" ::: "memory");
-        __syncthreads();                                                     // previous segment done everywhere: rings and exchange are free
-        F::tile_copy(c, 0, 0);
-        F::tile_copy(c, 1, 1);
-        for (int i = 0; i < c.nsteps; i += 3) {
+        if (tid == 0)
+            for (int i = i0; i < i0 + F_RING - 1 && i < c.nsteps; ++i) F::issue(c, i, i - i0);
+        for (int i = i0; i < c.nsteps; i += 3) {
             if (i >= c.st_lo && i + 3 <= c.st_hi) {
                 F::template step<0, true>(i, h, c);
                 F::template step<1, true>(i + 1, h, c);
@@ -508,16 +567,15 @@ __global__ void __launch_bounds__(512, 1) k_diffuse_tiled(const FusedArgs A, con
         }
         c.itg += (uint32_t)c.nsteps;
     }
-    asm volatile("cp.async.wait_group 0;" ::: "memory");
 }
 
 // ------------------------------------------------------------------ host side --
 struct FusedPlan {
     bool ok = false;
     int lrp = 0, sms = 0, fixed = 0;   // fixed: 0 run-time dims, 32 / 64: the cubic fast instantiations
-    bool tiled = false;                // planes wider than 64 sites: k_diffuse_tiled
+    bool tiled = false;                // planes wider or taller than 64 sites: k_diffuse_slab
+    int slab_warps = 0;
     bool writes_map = false;           // the kernel writes the S2/S3 occupancy map while the state planes pass through it
-    int tile_warps = 0;
     FusedArgs args{};
     int npass = 0, pass_nl[2] = { 0, 0 };
     // per context (= per device and host thread): shared-memory opt-in done, and the last split table, by NL
@@ -610,45 +668,63 @@ inline cudaError_t fused_launch_t(FusedPlan &F, const FusedArgs &A, int grid, cu
     return cudaGetLastError();
 }
 
-template <int NL, int NXG, int NYG>
-inline cudaError_t fused_launch_tiled_t(FusedPlan &F, const FusedArgs &A, int grid, cudaStream_t st)
+// shared-memory layout of the slab variant: rings sized for the tallest slab (rga row groups), y-exchange of whole lattice
+// rows, x-seam exchange
+inline size_t slab_smem(int nx, int nl, int rga, int nxb, FusedGeom &G)
+{
+    const int H = rga * F_PY;
+    size_t o = 128;
+    G.off_lut = (uint32_t)o; o += 96 * 4; o = (o + 127) / 128 * 128;
+    G.off_in = (uint32_t)o; o += (size_t)F_RING * H * nx * 4; o = (o + 127) / 128 * 128;
+    G.off_st = (uint32_t)o; o += (size_t)F_SRING * H * nx; o = (o + 127) / 128 * 128;
+    G.off_ex = (uint32_t)o; o += (size_t)2 * nl * 2 * (rga + 2) * nx * 4; o = (o + 127) / 128 * 128;
+    G.off_xex = (uint32_t)o; o += (size_t)2 * nl * (rga + 1) * nxb * 32; o = (o + 127) / 128 * 128;
+    G.smem_bytes = (uint32_t)o;
+    return o;
+}
+
+template <int NL, int LRP, int NXG, int NYG>
+inline cudaError_t fused_launch_slab_t(FusedPlan &F, const FusedArgs &A, int grid, cudaStream_t st)
 {
     FusedGeom G{};
-    fused_smem(64, 64, NL, 32, G);
-    G.nwarps = F.tile_warps;
-    const int units = A.batch * 3 * A.ntx * A.nty;
+    slab_smem(A.nx, NL, A.rga, A.nxb, G);
+    G.nwarps = F.slab_warps;
+    G.ngroups_alloc = A.rga;
+    const int units = A.batch * 3 * A.nslab;
     G.total_planes = (long long)units * (A.nz - 2);
     if (grid > F_MAXGRID) grid = F_MAXGRID;
     fused_split_cached(F, units, A.nz - 2, NL, grid, G.start);
     if (!F.attr_done[NL]) {
-        cudaError_t e = cudaFuncSetAttribute(k_diffuse_tiled<NL, NXG, NYG>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        cudaError_t e = cudaFuncSetAttribute(k_diffuse_slab<NL, LRP, NXG, NYG>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         if (e != cudaSuccess) return e;
         F.attr_done[NL] = true;
     }
-    k_diffuse_tiled<NL, NXG, NYG><<<grid, G.nwarps * 32, G.smem_bytes, st>>>(A, G);
+    k_diffuse_slab<NL, LRP, NXG, NYG><<<grid, G.nwarps * 32, G.smem_bytes, st>>>(A, G);
     return cudaGetLastError();
 }
 
 template <int NL>
-inline cudaError_t fused_launch_tiled(FusedPlan &F, const FusedArgs &A, int grid, cudaStream_t st)
+inline cudaError_t fused_launch_slab(FusedPlan &F, const FusedArgs &A, int grid, cudaStream_t st)
 {
-    if (A.nx == 96 && A.ny == 96) return fused_launch_tiled_t<NL, 96, 96>(F, A, grid, st);    // BASELINE configs[2]
-    if (A.nx == 80 && A.ny == 80) return fused_launch_tiled_t<NL, 80, 80>(F, A, grid, st);    // BASELINE configs[3]
-    return fused_launch_tiled_t<NL, 0, 0>(F, A, grid, st);
+    if (A.nx == 96 && A.ny == 96) return fused_launch_slab_t<NL, 16, 96, 96>(F, A, grid, st);    // BASELINE configs[2]
+    if (A.nx == 80 && A.ny == 80) return fused_launch_slab_t<NL, 8, 80, 80>(F, A, grid, st);     // BASELINE configs[3]
+    if (F.lrp == 32) return fused_launch_slab_t<NL, 32, 0, 0>(F, A, grid, st);
+    if (F.lrp == 16) return fused_launch_slab_t<NL, 16, 0, 0>(F, A, grid, st);
+    return fused_launch_slab_t<NL, 8, 0, 0>(F, A, grid, st);
 }
 
-// cut one lattice dimension into tiles of at most 64 sites including a halo of F_MAXNL towards neighbours; align: cuts on multiples of 4
-inline int fused_tiles(int n, short *t0, short *t1, short *o0, short *o1)
+// cut ny rows into slabs of at most H rows including a halo of F_MAXNL rows towards neighbours; cuts on multiples of F_PY
+inline int slab_cuts(int ny, int H, short *y0, short *y1, short *o0, short *o1)
 {
-    for (int nt = 1; nt <= 4; ++nt) {
+    for (int n = 1; n <= F_MAXSLAB; ++n) {
         bool ok = true;
-        for (int t = 0; t < nt && ok; ++t) {
-            const int c0 = t == 0 ? 0 : (n * t / nt) / 4 * 4, c1 = t == nt - 1 ? n : (n * (t + 1) / nt) / 4 * 4;
-            t0[t] = (short)std::max(0, c0 - F_MAXNL); t1[t] = (short)std::min(n, c1 + F_MAXNL);
+        for (int t = 0; t < n && ok; ++t) {
+            const int c0 = t == 0 ? 0 : (ny * t / n) / F_PY * F_PY, c1 = t == n - 1 ? ny : (ny * (t + 1) / n) / F_PY * F_PY;
+            y0[t] = (short)(t == 0 ? 0 : c0 - F_MAXNL); y1[t] = (short)(t == n - 1 ? ny : c1 + F_MAXNL);
             o0[t] = (short)c0; o1[t] = (short)c1;
-            ok = t1[t] - t0[t] <= 64 && c1 > c0;
+            ok = y1[t] - y0[t] <= H && c1 > c0 && y0[t] >= 0 && y1[t] <= ny && y1[t] - y0[t] >= 2 * F_PY;
         }
-        if (ok) return nt;
+        if (ok) return n;
     }
     return 0;
 }
@@ -656,7 +732,7 @@ inline int fused_tiles(int n, short *t0, short *t1, short *o0, short *o1)
 template <int NL>
 inline cudaError_t fused_launch_nl(FusedPlan &F, const FusedArgs &A, int grid, cudaStream_t st)
 {
-    if (F.tiled) return fused_launch_tiled<NL>(F, A, grid, st);
+    if (F.tiled) return fused_launch_slab<NL>(F, A, grid, st);
     if (F.fixed == 64) return fused_launch_t<NL, 32, 64, 64>(F, A, grid, st);
     if (F.fixed == 32) return fused_launch_t<NL, 16, 32, 32>(F, A, grid, st);
     if (F.lrp == 16) return fused_launch_t<NL, 16, 0, 0>(F, A, grid, st);
@@ -669,20 +745,30 @@ inline void fused_configure(const KParams &P, FusedPlan &F)
     F.ok = false;
     F.tiled = (P.nx > 64 || P.ny > 64);
     if (P.nz < 3 || P.n_sub < 1 || P.n_sub > 2 * F_MAXNL || P.nx < 4) return;
-    if (F.tiled) {
-        if (P.nx % 4 || P.ny % 4) return;                         // aligned copies; tiles are whole strips of 4 rows                                    // 4-byte state copies and 8-byte field copies must stay aligned
-        F.args.ntx = fused_tiles(P.nx, F.args.tx0, F.args.tx1, F.args.ox0, F.args.ox1);
-        F.args.nty = fused_tiles(P.ny, F.args.ty0, F.args.ty1, F.args.oy0, F.args.oy1);
-        if (!F.args.ntx || !F.args.nty) return;
-        int maxh = 0;
-        for (int t = 0; t < F.args.nty; ++t) maxh = std::max(maxh, F.args.ty1[t] - F.args.ty0[t]);
-        F.tile_warps = (maxh + F_PY - 1) / F_PY;
-    } else if (P.nx % 2 || (P.nx * P.ny) % 16) return;
-    F.lrp = P.nx <= 32 ? 16 : 32;
-    F.fixed = (P.nx == 64 && P.ny == 64) ? 64 : (P.nx == 32 && P.ny == 32) ? 32 : 0;
-    F.writes_map = F.fixed != 0 && !F.tiled;
     FusedGeom G{};
-    if (!F.tiled && (fused_smem(P.nx, P.ny, F_MAXNL, F.lrp, G) > 227 * 1024 || G.nwarps > 16)) return;
+    if (F.tiled) {
+        // rows must be whole 16-byte units of the state array (bulk copies) and whole row groups of 2 * LRP sites
+        if (P.nx % 16 || P.ny % F_PY) return;
+        F.lrp = P.nx % 64 == 0 ? 32 : (P.nx % 32 == 0 ? 16 : 8);
+        const int rw = 32 / F.lrp;
+        F.args.nxb = P.nx / (2 * F.lrp);
+        F.args.rga = (16 * rw) / F.args.nxb;                      // row groups of F_PY rows that 16 warps hold
+        if (F.args.rga < 3) return;
+        F.args.nslab = slab_cuts(P.ny, F.args.rga * F_PY, F.args.sy0, F.args.sy1, F.args.so0, F.args.so1);
+        if (!F.args.nslab) return;
+        int maxh = 0;
+        for (int t = 0; t < F.args.nslab; ++t) maxh = std::max(maxh, F.args.sy1[t] - F.args.sy0[t]);
+        F.slab_warps = ((maxh / F_PY) * F.args.nxb + rw - 1) / rw;   // the tallest slab decides the CTA size (the rings keep their capacity)
+        if (slab_smem(P.nx, F_MAXNL, F.args.rga, F.args.nxb, G) > 227 * 1024 || F.slab_warps > 16) return;
+        F.fixed = 0;
+        F.writes_map = (P.nx * P.ny) % 256 == 0;                  // occupancy words must not straddle planes
+    } else {
+        if (P.nx % 2 || (P.nx * P.ny) % 16) return;
+        F.lrp = P.nx <= 32 ? 16 : 32;
+        F.fixed = (P.nx == 64 && P.ny == 64) ? 64 : (P.nx == 32 && P.ny == 32) ? 32 : 0;
+        F.writes_map = F.fixed != 0;
+        if (fused_smem(P.nx, P.ny, F_MAXNL, F.lrp, G) > 227 * 1024 || G.nwarps > 16) return;
+    }
     int dev = 0;
     cudaDeviceProp prop;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return;

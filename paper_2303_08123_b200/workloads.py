@@ -19,7 +19,10 @@ MASTER_SEED = 230308123
 
 # Default parameter set ("O-PARAM").  Medium values are the
 # paper's (glucose 5.5 mM, O2 0.28 mM, pH 7.4 -> [H+] 3.98e-5 mM);
-# 600 steps/h is PAPER.md l.262.  Everything else is this build's reading.
+# 600 steps/h is PAPER.md l.262.  Everything else is this build's reading.  The uptake / production rates were tuned once
+# (round 2) against pin P12 at BASELINE configs[2] size -- a spheroid grown from one cell to 64 sites across on 96^3 shows a
+# proliferating rim (mean radius 22.8 sites), a quiescent shell (16.2) and a necrotic, partly lysed core (dead cells at
+# 12.5, ~6900 vacated sites inside half the radius) -- and are frozen since.
 _DEFAULT = {
     "steps_per_hour": 600,
     "n_sub": 4,
@@ -27,9 +30,9 @@ _DEFAULT = {
     "boundary": [0.28, 5.5, 3.98e-5],
     # signed source per sub-step [species][mode PA, PN, QA, QN]
     "rate": [
-        [-4e-4, 0.0, -2e-4, 0.0],                  # O2 uptake
-        [-8e-4, -2.4e-3, -4e-4, -1.2e-3],          # glucose uptake
-        [1.5e-8, 6e-8, 0.75e-8, 3e-8],             # H+ production
+        [-6e-4, 0.0, -3e-4, 0.0],                  # O2 uptake
+        [-1.2e-3, -3.6e-3, -6e-4, -1.8e-3],        # glucose uptake
+        [2.25e-8, 9e-8, 1.125e-8, 4.5e-8],         # H+ production
     ],
     "O_A": 0.02, "G_P": 0.5, "G_Q": 0.05, "H_P": 1.58e-4, "H_Q": 3.98e-4,
     "T": [3000, 4800, 1800, 600],                  # G1, S, G2, M  (17 h cycle, PAPER.md l.196/l.232 hint)
@@ -133,6 +136,20 @@ def config(k):
                     init=dict(kind="ball", center=(32, 32, 32), radius=9.0, shared_init=True),
                     warmup_h=6.0, t0_h=6.0, horizon_h=720.0, dose=dose, delay=delay, nfrac=nfrac)
     raise ValueError("config index must be 1..5")
+
+
+def reduced_c2():
+    """Reduced BASELINE configs[1] job for long-horizon statistical parity (SURVEY 8(c) protocol (3)): what the fp64 oracle
+    can afford on the host cores.  32^3 lattice, shared BALL r = 4 (257 cells), 6 h warm-up, 8 protocols of 4 fractions
+    (configs[1] dose alphabet, delays 6..24 h so that the treatment fits the 5-day horizon), 30 seeds each."""
+    seed = MASTER_SEED + 12
+    rng = np.random.default_rng(seed)
+    npro, nfr = 8, 4
+    dose = DOSE_ALPHABET[rng.integers(0, len(DOSE_ALPHABET), (npro, nfr))]
+    delay = 6.0 * (1 + rng.integers(0, 4, (npro, nfr)))
+    return dict(name="c2-reduced", population=npro, seeds_per_protocol=30, batch=npro * 30, dims=(32, 32, 32), rng_seed=seed,
+                sim_id_base=0, init=dict(kind="ball", center=(16, 16, 16), radius=4.0, shared_init=True),
+                warmup_h=6.0, t0_h=6.0, horizon_h=120.0, dose=dose, delay=delay, nfrac=np.full(npro, nfr, np.int32))
 
 
 def robustness_sweep(base_dose, base_delay, shifts_h=(-1.0, -0.5, 0.5, 1.0), step_h=0.5):

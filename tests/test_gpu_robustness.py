@@ -113,7 +113,7 @@ def test_step_aligned_fp32_delays_are_accepted_and_fire_on_the_oracle_steps():
     r = o.OracleSim(16, 16, 16, p)
     r.seed("single", rng_seed=1)
     r.set_protocol(dose[0], delay[0])
-    assert r.fire_steps() == [210, 630, 4290, 4293]
+    assert r.fire_steps().tolist() == [210, 630, 4290, 4293]
     g.step(215)                                  # crosses the first fraction
     r.step(215)
     assert_ints_equal(g.get_state(0), r.get_state(), "after fraction 0")

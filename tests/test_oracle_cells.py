@@ -228,3 +228,32 @@ def test_p12_untreated_growth_is_monotone_and_compact():
     r = np.sqrt((zz - 10) ** 2 + (yy - 10) ** 2 + (xx - 10) ** 2)
     r_eq = (3 * last / (4 * np.pi)) ** (1 / 3)
     assert r.max() < 1.8 * r_eq + 2                  # roughly spherical, no streamers
+
+
+def test_p12_radial_order_rim_quiescent_shell_necrotic_core():
+    """Pin P12, qualitative (SURVEY c.7; "a proliferating rim", quiescence, "progression of necrosis"):
+    an untreated spheroid that outgrows its nutrient supply shows, from outside to inside, proliferating cells, a
+    quiescent shell and a necrotic core that hollows out by lysis.  Scaled-down scenario (short cycle, uptake x16, so
+    the viable depth is ~5 sites on a 30^3 lattice); the same order is checked on the GPU at BASELINE configs[2] size
+    (tests/test_gpu_long.py).  Numbers are not the paper's: parity unpinned, sanity only."""
+    n = 30
+    p = w.default_params(T=[60, 96, 36, 12], J=[6, 10, 4, 1], lysis_steps=400)
+    p["rate"] = [[16.0 * r for r in row] for row in p["rate"]]
+    sim = o.OracleSim(n, n, n, p)
+    sim.seed("cluster7", rng_seed=77)
+    sim.step(2400)
+    st = sim.get_state()["state"]
+    k = st & 7
+    lv = (k >= 1) & (k <= 4)
+    mode = (st >> 3) & 3
+    zz, yy, xx = np.indices(st.shape)
+    occ = lv | (k == 5)
+    c = [a[occ].mean() for a in (zz, yy, xx)]
+    r = np.sqrt((zz - c[0]) ** 2 + (yy - c[1]) ** 2 + (xx - c[2]) ** 2)
+    prolif, quiet, dead = lv & (mode < 2), lv & (mode >= 2), k == 5
+    assert prolif.sum() > 300 and quiet.sum() > 100 and dead.sum() > 50
+    assert r[prolif].mean() > r[quiet].mean() + 0.8 > r[dead].mean() + 1.6
+    anaerobic = lv & ((mode & 1) == 1)
+    assert r[anaerobic].mean() < r[lv & ((mode & 1) == 0)].mean()                 # oxygen runs out from the inside
+    assert ((k == 0) & (r < 0.4 * r[occ].max())).sum() > 20                       # lysed core
+    assert abs(c[0] - 15) < 1.5 and abs(c[1] - 15) < 1.5 and abs(c[2] - 15) < 1.5  # stays centred
