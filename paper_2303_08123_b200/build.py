@@ -29,7 +29,7 @@ def build(force=False, verbose=False):
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(s) for s in srcs):
         return LIB
     nvcc = os.environ.get("NVCC", "nvcc")
-    cmd = [nvcc, *NVCC_FLAGS, "-o", LIB, os.path.join(CSRC, "ca_api.cu")]
+    cmd = [nvcc, *NVCC_FLAGS, *os.environ.get("CA_NVCC_EXTRA", "").split(), "-o", LIB, os.path.join(CSRC, "ca_api.cu")]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
     subprocess.check_call(cmd)

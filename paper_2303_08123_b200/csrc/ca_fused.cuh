@@ -38,6 +38,7 @@ constexpr int F_RING = 3;      // field-plane ring depth = register phase count 
 constexpr int F_SRING = 8;     // state-plane ring depth (a plane is used by NL consecutive iterations)
 constexpr int F_MAXNL = 4;
 constexpr int F_MAXSLAB = 8;
+constexpr int F_SLAB_WARPS = 15;  // slab variant: 480 threads, so that a thread may use 136 registers (the seam exchange needs a few more than 128)
 constexpr int F_MAXGRID = 640; // persistent CTAs at most (the split table travels as a kernel parameter)
 
 struct FusedArgs {
@@ -106,7 +107,7 @@ __device__ __forceinline__ void sts128f(uint32_t a, float x, float y, float z, f
 
 struct FusedGeom {             // host-computed launch geometry, passed by value
     int nwarps, ngroups_alloc; // strips of F_PY rows: groups = nwarps * (32 / LRP)
-    uint32_t off_lut, off_in, off_st, off_ex, off_xex, smem_bytes;
+    uint32_t off_lut, off_in, off_st, off_ex, off_xex, off_xdummy, smem_bytes;
     long long total_planes;    // batch * 3 * (nz - 2): the flattened (unit, interior plane) space
     int start[F_MAXGRID + 1];  // CTA g works on flattened planes [start[g], start[g+1]) (cost-balanced on the host)
 };
@@ -136,13 +137,22 @@ struct FusedCtx {
     uint32_t *occ_row;         // species 0 only: occupancy words of this warp's strip, indexed by plane (else NULL)
     // slab variant
     uint32_t in_slot, st_slot;     // bytes of one ring slot (the tallest slab)
-    uint32_t ld_fbytes, ld_sbytes; // bytes of this slab's rows of a field / state plane
     uint32_t yst;                  // bytes of one row of the y-exchange (a whole lattice row)
-    uint32_t xs_w, xs_r, xel;      // x-seam exchange between column blocks: my store / load slot (buffer 0, level 0), bytes per level
-    bool seam, seam_r;             // this lane sits on a seam between two column blocks; ... on the right edge of its block
-    uint32_t occ_w0, occ_nw;       // species 0: occupancy words of a plane this slab is responsible for
-    uint32_t occ_soff;             // byte offset of word occ_w0 inside the state slot (may wrap negative never: halo covers it)
+    uint32_t xs_w, xel;            // x-seam exchange between column blocks: my store slot (buffer 0, level 0), bytes per level
+    bool seam_l, seam_r;           // this lane sits on a seam between two column blocks, on the left / right edge of its block
+    uint32_t occ_nw;               // species 0: number of occupancy words of a plane this slab is responsible for (else 0)
 };
+
+// slab variant: per-segment constants that only the producer thread (bulk copies) or one lane per warp (occupancy words) needs
+// live in shared memory, not in registers
+struct SlabSeg {
+    const float *src_plane0;       // first loaded row of plane 0 of this unit
+    const uint8_t *st_plane0;
+    uint32_t *occ_row;             // occupancy words of this simulation
+    uint32_t ld_fbytes, ld_sbytes; // bytes of this slab's rows of a field / state plane
+    uint32_t occ_w0, occ_soff;     // first word this slab writes; its byte offset inside the state slot
+};
+constexpr uint32_t F_SEG_OFF = 32; // inside the first 128 bytes of shared memory, after the mbarriers
 
 // NX = NY = 0: lattice dims at run time (any even nx <= 2*LRP); otherwise compile-time dims, all address math folds
 // SLAB: planes larger than a CTA holds; NX, NY then give the lattice (NX = nxb * 2 * LRP) and the CTA works on y-slabs
@@ -151,7 +161,7 @@ struct Fused {
     static constexpr bool FIXED = NX != 0;
     static constexpr int RW = 32 / LRP;
     static constexpr int NXB = (SLAB && FIXED) ? NX / (2 * LRP) : 1;                 // column blocks (slab variant with compile-time dims)
-    static constexpr int RGA = (SLAB && FIXED) ? (16 * RW) / NXB : 0;                // row groups a CTA of 16 warps holds
+    static constexpr int RGA = (SLAB && FIXED) ? (F_SLAB_WARPS * RW) / NXB : 0;      // row groups a CTA of 15 warps holds
     // every lane and row holds valid data: whole fixed-size planes, or a slab (groups beyond a short slab are clamped onto its
     // last row group: they compute duplicates that feed only the frozen last row and are never stored)
     static constexpr bool FULL = SLAB || (FIXED && NX == 2 * LRP && NY % (F_PY * RW) == 0);
@@ -204,16 +214,20 @@ struct Fused {
     // slab variant: a lane on a seam publishes its edge column (F_PY rows) of level K for the neighbouring column block
     static __device__ __forceinline__ void seam_store(const FusedCtx &c, const uint32_t addr, const u64 (&V)[F_PY])
     {
-        if (c.seam) {
-            float e[F_PY];
+        float e[F_PY];                                                      // no branch: lanes off a seam store into a sink slot
 #pragma unroll
-            for (int j = 0; j < F_PY; ++j) {
-                float a, b;
-                upk(V[j], a, b);
-                e[j] = c.seam_r ? b : a;
-            }
-            sts128f(addr, e[0], e[1], e[2], e[3]);
+        for (int j = 0; j < F_PY; ++j) {
+            float a, b;
+            upk(V[j], a, b);
+            e[j] = c.seam_r ? b : a;
         }
+        sts128f(addr, e[0], e[1], e[2], e[3]);
+    }
+
+    static __device__ __forceinline__ SlabSeg *slab_seg()
+    {
+        extern __shared__ __align__(128) unsigned char fsm_[];
+        return reinterpret_cast<SlabSeg *>(fsm_ + F_SEG_OFF);
     }
 
     // producer (one thread): start the bulk copies of iteration i into field-ring slot i mod 3
@@ -221,11 +235,17 @@ struct Fused {
     {
         const int t = c.t0 + i;
         const uint32_t bar = c.bars + 8u * (uint32_t)slot;
-        const uint32_t pb = SLAB ? c.ld_fbytes : (uint32_t)nxny(c) * 4u, sb = SLAB ? c.ld_sbytes : (uint32_t)nxny(c);   // a slab's rows are contiguous
         if (t >= c.ld_lo && t < c.ld_hi) {
+            uint32_t pb = (uint32_t)nxny(c) * 4u, sb = (uint32_t)nxny(c);
+            const float *fsrc = c.src_plane0;
+            const uint8_t *ssrc = c.st_plane0;
+            if constexpr (SLAB) {                                            // a slab's rows are contiguous; its constants live in shared memory
+                const SlabSeg *sg = slab_seg();
+                pb = sg->ld_fbytes; sb = sg->ld_sbytes; fsrc = sg->src_plane0; ssrc = sg->st_plane0;
+            }
             mbar_expect_tx(bar, pb + sb);
-            bulk_g2s(c.in_ring + (uint32_t)slot * inslot(c), c.src_plane0 + (size_t)t * nxny(c), pb, bar);
-            bulk_g2s(c.st_ring + ((c.itg + (uint32_t)i) & (F_SRING - 1)) * stslot(c), c.st_plane0 + (size_t)t * nxny(c), sb, bar);
+            bulk_g2s(c.in_ring + (uint32_t)slot * inslot(c), fsrc + (size_t)t * nxny(c), pb, bar);
+            bulk_g2s(c.st_ring + ((c.itg + (uint32_t)i) & (F_SRING - 1)) * stslot(c), ssrc + (size_t)t * nxny(c), sb, bar);
         } else {
             mbar_arrive(bar);
         }
@@ -248,11 +268,11 @@ struct Fused {
                 const u64 dn = lds64(exr + (uint32_t)(K - 1) * el + yst(c));             // top row of the strip below
                 float4 xe = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
                 if constexpr (SLAB) {
-                    if (c.seam) xe = lds128f(xsr + (uint32_t)(K - 1) * xel(c));                  // the neighbour block's edge column, written by the previous iteration
+                    xe = lds128f(xsr + (uint32_t)(K - 1) * xel(c));                             // the neighbour block's edge column, written by the previous iteration (lanes off a seam: a sink nobody selects from)
                 }
                 u64 nloc[F_PY];
                 u64 (&N)[F_PY] = *(K < NL ? &h[KO][sc] : &nloc);
-                level(h[K - 1][sm], h[K - 1][sc], h[K - 1][sp], N, up, dn, c.lam2, c.zero2, xe, c.seam && !c.seam_r, c.seam_r);
+                level(h[K - 1][sm], h[K - 1][sc], h[K - 1][sp], N, up, dn, c.lam2, c.zero2, xe, c.seam_l, c.seam_r);
                 if (!NOCELLS && (((c.flags | c.slowmask) >> K) & 1u)) {    // cells in this strip: source term and clamp
                     const uint32_t s = c.st_lane + ((q - (uint32_t)K) & (F_SRING - 1)) * stslot(c);
 #pragma unroll
@@ -313,10 +333,10 @@ struct Fused {
         const uint32_t exw = c.ex_self + ((uint32_t)i & 1u) * exb;          // rows written now, read by the next iteration
         const uint32_t exr = c.ex_self + exb - ((uint32_t)i & 1u) * exb;    // rows written by the previous iteration
         uint32_t xsw = 0, xsr = 0;
-        if constexpr (SLAB) {
+        if constexpr (SLAB) {                                                // the facing slot of the neighbour block is the next / previous 16 bytes
             const uint32_t xb = xel(c) * NL;
             xsw = c.xs_w + ((uint32_t)i & 1u) * xb;
-            xsr = c.xs_r + xb - ((uint32_t)i & 1u) * xb;
+            xsr = c.xs_w + xb - ((uint32_t)i & 1u) * xb + (c.seam_r ? 16u : 0xFFFFFFF0u);
         }
         // ---- level 0: plane t from the ring
         mbar_wait(c.bars + 8u * PH, (c.par >> PH) & 1u);
@@ -331,19 +351,16 @@ struct Fused {
             if constexpr (SLAB) seam_store(c, xsw, h[0][PH]);
             // "cells in my strip": every lane looks at 8 bytes of the warp's strip of the state plane; a byte counts when kind is 1..6
             if constexpr (SLAB) {                                            // a warp's points are not contiguous bytes: every lane looks at its own 2 x 4 bytes
-                const uint32_t sa = c.st_lane + (q & (F_SRING - 1)) * stslot(c);
-                uint32_t m = 0;
-#pragma unroll
-                for (int j = 0; j < F_PY; ++j) m |= ((lds16(sa + (uint32_t)j * stpitch(c)) & 0x0707u) + 0x0101u) & 0x0606u;
-                any = m != 0u;
+                // the warp's points are 32 / LRP row groups x F_PY rows x 2 * LRP contiguous bytes: every lane looks at 8 of them
+                const u64 wv = lds64(c.st_strip + (q & (F_SRING - 1)) * stslot(c));
+                any = (((wv & 0x0707070707070707ull) + 0x0101010101010101ull) & 0x0606060606060606ull) != 0ull;
                 // the S2/S3 occupancy map (one bit per 8 consecutive state bytes, one word per 256): this slab's words of the plane,
                 // read from the state slab in shared memory, one word per warp and trip
-                if (c.occ_row != nullptr) {
-                    for (uint32_t w = threadIdx.x >> 5; w < c.occ_nw; w += blockDim.x >> 5) {
-                        const u64 v = lds64(c.st_ring + (q & (F_SRING - 1)) * stslot(c) + c.occ_soff + w * 256u + 8u * (threadIdx.x & 31u));
-                        const uint32_t bal = __ballot_sync(0xFFFFFFFFu, (((v & 0x0707070707070707ull) + 0x0101010101010101ull) & 0x0606060606060606ull) != 0ull);
-                        if ((threadIdx.x & 31) == 0) c.occ_row[(size_t)t * (size_t)(nxny(c) / 256) + c.occ_w0 + w] = bal;
-                    }
+                for (uint32_t w = threadIdx.x >> 5; w < c.occ_nw; w += blockDim.x >> 5) {
+                    const SlabSeg *sg = slab_seg();
+                    const u64 v = lds64(c.st_ring + (q & (F_SRING - 1)) * stslot(c) + sg->occ_soff + w * 256u + 8u * (threadIdx.x & 31u));
+                    const uint32_t bal = __ballot_sync(0xFFFFFFFFu, (((v & 0x0707070707070707ull) + 0x0101010101010101ull) & 0x0606060606060606ull) != 0ull);
+                    if ((threadIdx.x & 31) == 0) sg->occ_row[(size_t)t * (size_t)(nxny(c) / 256) + sg->occ_w0 + w] = bal;
                 }
             } else {
                 const u64 w = c.strip_ok ? lds64(c.st_strip + (q & (F_SRING - 1)) * (uint32_t)nxny(c)) : 0ull;
@@ -465,14 +482,14 @@ __global__ void __launch_bounds__(512, 1) k_diffuse_fused(const FusedArgs A, con
 // y-neighbours across row groups.  The S2/S3 occupancy map is written from the state slab while it is in shared memory.
 // NXG, NYG: lattice dims at compile time (all strides fold); 0 = run time.
 template <int NL, int LRP, int NXG, int NYG>
-__global__ void __launch_bounds__(512, 1) k_diffuse_slab(const FusedArgs A, const FusedGeom Gm)
+__global__ void __launch_bounds__(F_SLAB_WARPS * 32, 1) k_diffuse_slab(const FusedArgs A, const FusedGeom Gm)
 {
     typedef Fused<NL, LRP, NXG, NYG, true> F;
     extern __shared__ __align__(128) unsigned char fsm[];
     constexpr int RW = 32 / LRP;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int lx = lane % LRP, gi = warp * RW + lane / LRP;
-    const int nxb = NXG ? NXG / (2 * LRP) : A.nxb, rga = NXG ? (16 * RW) / (NXG / (2 * LRP)) : A.rga;
+    const int nxb = NXG ? NXG / (2 * LRP) : A.nxb, rga = NXG ? (F_SLAB_WARPS * RW) / (NXG / (2 * LRP)) : A.rga;
     const int blk = gi % nxb, rg = gi / nxb;                                  // column block, row group inside the slab
     const int nxr = NXG ? NXG : A.nx, nyr = NYG ? NYG : A.ny;
     const int x0 = blk * 2 * LRP + 2 * lx;
@@ -487,10 +504,12 @@ __global__ void __launch_bounds__(512, 1) k_diffuse_slab(const FusedArgs A, cons
     c.ex_self = base + Gm.off_ex + (uint32_t)(rg + 1) * c.yst + (uint32_t)x0 * 4u;
     c.xel = (uint32_t)(rga * nxb) * 32u;                                       // per level: [row group][block][left edge | right edge] x 16 bytes
     c.seam_r = lx == LRP - 1 && blk < nxb - 1;
-    c.seam = c.seam_r || (lx == 0 && blk > 0);
+    c.seam_l = lx == 0 && blk > 0;
+    // slots: [row group][block][left edge | right edge] x 16 bytes, so the facing edge of the neighbour block is the slot before / after mine;
+    // lanes off a seam all use the first slot of a sink region of the same shape (written, read, never selected)
     c.xs_w = base + Gm.off_xex + (uint32_t)((rg * nxb + blk) * 2 + (c.seam_r ? 1 : 0)) * 16u;
-    c.xs_r = base + Gm.off_xex + (uint32_t)((rg * nxb + blk + (c.seam_r ? 1 : -1)) * 2 + (c.seam_r ? 0 : 1)) * 16u;   // the neighbour block's facing edge
-    c.st_strip = 0; c.strip_ok = false;
+    if (!c.seam_l && !c.seam_r) c.xs_w = base + Gm.off_xdummy + 16u;
+    c.st_strip = 0; c.strip_ok = true; c.src_plane0 = nullptr; c.st_plane0 = nullptr; c.occ_row = nullptr;
     c.itg = 0; c.par = 0;
     c.zero2 = pk(A.zero, A.zero);
     if (tid == 0) {
@@ -524,24 +543,34 @@ __global__ void __launch_bounds__(512, 1) k_diffuse_slab(const FusedArgs A, cons
         const int y0 = ty0 + F_PY * rg;
         const int yc = min(y0, ty1 - F_PY);                                    // groups beyond a short slab: duplicates of its last row group
         const size_t ubase = (size_t)b * (size_t)c.nxny * (size_t)A.nz;
-        c.src_plane0 = A.src[sp] + ubase + (size_t)ty0 * nxr;
-        c.st_plane0 = A.state + ubase + (size_t)ty0 * nxr;
-        c.ld_fbytes = (uint32_t)((ty1 - ty0) * nxr) * 4u; c.ld_sbytes = (uint32_t)((ty1 - ty0) * nxr);
+        c.occ_nw = 0;
+        if (sp == 0 && A.occ != nullptr) c.occ_nw = (uint32_t)((oy1 * nxr + 255) / 256) - (uint32_t)((oy0 * nxr + 255) / 256);
+        if (tid == 0) {                                                        // every reader of the old values is past the last barrier of the previous segment
+            SlabSeg *sg = F::slab_seg();
+            sg->src_plane0 = A.src[sp] + ubase + (size_t)ty0 * nxr;
+            sg->st_plane0 = A.state + ubase + (size_t)ty0 * nxr;
+            sg->ld_fbytes = (uint32_t)((ty1 - ty0) * nxr) * 4u; sg->ld_sbytes = (uint32_t)((ty1 - ty0) * nxr);
+            // occupancy words of a plane whose first byte lies in this slab's output rows (the halo covers the rest of the word)
+            sg->occ_row = A.occ ? A.occ + (size_t)b * (size_t)(c.nxny / 256) * (size_t)A.nz : nullptr;
+            sg->occ_w0 = (uint32_t)((oy0 * nxr + 255) / 256);
+            sg->occ_soff = sg->occ_w0 * 256u - (uint32_t)(ty0 * nxr);
+        }
+        __syncthreads();
         c.src = A.src[sp] + ubase + (yc * nxr + x0);
         c.dst = A.dst[sp] + ubase + (yc * nxr + x0);
         c.in_lane = c.in_ring + (uint32_t)((yc - ty0) * nxr + x0) * 4u;
         c.st_lane = c.st_ring + (uint32_t)((yc - ty0) * nxr + x0);
+        {   // segment = one row of one row group of this warp: LRP / 4 lanes x 8 bytes
+            const int seg = lane / (LRP / 4), sg_g = warp * RW + seg / F_PY, sg_row = seg % F_PY;
+            const int sy = min(ty0 + F_PY * (sg_g / nxb), ty1 - F_PY) + sg_row;
+            c.st_strip = c.st_ring + (uint32_t)((sy - ty0) * nxr + (sg_g % nxb) * 2 * LRP + (lane % (LRP / 4)) * 8);
+        }
         c.t0 = c.za - NL;
         c.nsteps = c.zb - c.za + 2 * NL;
         c.ld_lo = max(0, c.za - NL); c.ld_hi = min(A.nz, c.zb + NL);
         c.st_lo = 2 * NL; c.st_hi = min(A.nz, c.zb + NL) - c.t0;
         c.flags = 0; c.slowmask = A.always_slow[sp] ? 0xFFFFFFFFu : 0u;
         c.lut = base + Gm.off_lut + (uint32_t)sp * 128u;
-        // occupancy words of a plane whose first byte lies in this slab's output rows (the halo covers the rest of the word)
-        c.occ_row = (sp == 0 && A.occ != nullptr) ? A.occ + (size_t)b * (size_t)(c.nxny / 256) * (size_t)A.nz : nullptr;
-        c.occ_w0 = (uint32_t)((oy0 * nxr + 255) / 256);
-        c.occ_nw = (uint32_t)((oy1 * nxr + 255) / 256) - c.occ_w0;
-        c.occ_soff = c.occ_w0 * 256u - (uint32_t)(ty0 * nxr);
         const float lam = A.lam[sp];
         c.rowmask = 0;
 #pragma unroll
@@ -679,6 +708,7 @@ inline size_t slab_smem(int nx, int nl, int rga, int nxb, FusedGeom &G)
     G.off_st = (uint32_t)o; o += (size_t)F_SRING * H * nx; o = (o + 127) / 128 * 128;
     G.off_ex = (uint32_t)o; o += (size_t)2 * nl * 2 * (rga + 2) * nx * 4; o = (o + 127) / 128 * 128;
     G.off_xex = (uint32_t)o; o += (size_t)2 * nl * (rga + 1) * nxb * 32; o = (o + 127) / 128 * 128;
+    G.off_xdummy = (uint32_t)o; o += (size_t)2 * nl * (rga + 1) * nxb * 32 + 128;
     G.smem_bytes = (uint32_t)o;
     return o;
 }
@@ -752,14 +782,14 @@ inline void fused_configure(const KParams &P, FusedPlan &F)
         F.lrp = P.nx % 64 == 0 ? 32 : (P.nx % 32 == 0 ? 16 : 8);
         const int rw = 32 / F.lrp;
         F.args.nxb = P.nx / (2 * F.lrp);
-        F.args.rga = (16 * rw) / F.args.nxb;                      // row groups of F_PY rows that 16 warps hold
+        F.args.rga = (F_SLAB_WARPS * rw) / F.args.nxb;            // row groups of F_PY rows that 15 warps hold
         if (F.args.rga < 3) return;
         F.args.nslab = slab_cuts(P.ny, F.args.rga * F_PY, F.args.sy0, F.args.sy1, F.args.so0, F.args.so1);
         if (!F.args.nslab) return;
         int maxh = 0;
         for (int t = 0; t < F.args.nslab; ++t) maxh = std::max(maxh, F.args.sy1[t] - F.args.sy0[t]);
         F.slab_warps = ((maxh / F_PY) * F.args.nxb + rw - 1) / rw;   // the tallest slab decides the CTA size (the rings keep their capacity)
-        if (slab_smem(P.nx, F_MAXNL, F.args.rga, F.args.nxb, G) > 227 * 1024 || F.slab_warps > 16) return;
+        if (slab_smem(P.nx, F_MAXNL, F.args.rga, F.args.nxb, G) > 227 * 1024 || F.slab_warps > F_SLAB_WARPS) return;
         F.fixed = 0;
         F.writes_map = (P.nx * P.ny) % 256 == 0;                  // occupancy words must not straddle planes
     } else {
@@ -812,9 +842,11 @@ inline int launch_fused(FusedPlan &F, const Lattice &L, int cur, uint32_t *occ, 
         const int grid = (int)std::max<long long>(1, std::min<long long>((long long)F.sms * per_sm, total / 2 + 1));
         cudaError_t e;
         switch (F.pass_nl[ps]) {
+#ifndef CA_ONLY_NL4                     // development builds: only the n_sub = 4 instantiations (compile time)
         case 1: e = fused_launch_nl<1>(F, A, grid, st); break;
         case 2: e = fused_launch_nl<2>(F, A, grid, st); break;
         case 3: e = fused_launch_nl<3>(F, A, grid, st); break;
+#endif
         case 4: e = fused_launch_nl<4>(F, A, grid, st); break;
         default: e = cudaErrorInvalidValue;
         }
