@@ -429,7 +429,7 @@ def run_probe(args):
         if args.tumour_radius is not None:          # late-phase probe: the same lattice started from a larger seeded ball
             cfg["init"] = dict(cfg["init"], kind="ball", radius=float(args.tumour_radius))
         snap = warm_snapshot(binding, cfg, params, 0)
-    kern = "k_diffuse_fused" if k == 2 else "k_diffuse_slab"
+    kern = "k_diffuse_fused" if k == 2 else "k_diffuse_rows"
     out = config_probe(torch, binding, str(k - 1), cfg, params, snap, 0, args.ca_steps or (200 if k == 2 else 20), kern, None)
     out["probe"] = {"config": args.probe, "batch": cfg["batch"], "tumour_radius": args.tumour_radius}
     print(json.dumps(out))
@@ -560,12 +560,12 @@ def run_ours(args):
             c3 = w.config(3)
             snap3, grown_h = pregrow.grow(c3["dims"], params, c3["init"], c3["rng_seed"], target_extent=c3["pregrow_diameter"], check_h=24.0, device=local)
             c3["t0_h"] = grown_h
-            per_config["2"] = config_probe(torch, binding, "2", c3, params, snap3, local, 20, "k_diffuse_slab", "r*_ncu_slab_c3*.txt")
+            per_config["2"] = config_probe(torch, binding, "2", c3, params, snap3, local, 20, "k_diffuse_rows", "r*_ncu_rows_c3*.txt")
             per_config["2"]["pregrown_hours"] = grown_h
             per_config["2"]["pregrown_profile"] = pregrow.radial_profile(snap3)
             c4 = w.config(4)
             snap4 = warm_snapshot(binding, c4, params, local)
-            per_config["3"] = config_probe(torch, binding, "3", c4, params, snap4, local, 20, "k_diffuse_slab", "r*_ncu_slab_c4*.txt")
+            per_config["3"] = config_probe(torch, binding, "3", c4, params, snap4, local, 20, "k_diffuse_rows", "r*_ncu_rows_c4*.txt")
             if not args.skip_full_horizon:
                 fullh = full_horizon(torch, binding, c2, params, snap, local)
         if world == 1 and not args.no_cpu_baseline:

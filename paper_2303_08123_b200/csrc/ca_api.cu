@@ -11,6 +11,7 @@
 
 #include "ca_kernels.cuh"
 #include "ca_fused.cuh"
+#include "ca_rows.cuh"
 
 using namespace ca;
 

@@ -604,6 +604,7 @@ struct FusedPlan {
     int lrp = 0, sms = 0, fixed = 0;   // fixed: 0 run-time dims, 32 / 64: the cubic fast instantiations
     bool tiled = false;                // planes wider or taller than 64 sites: k_diffuse_slab
     int slab_warps = 0;
+    bool rows = false;                 // k_diffuse_rows (ca_rows.cuh) covers this width; else k_diffuse_slab
     bool writes_map = false;           // the kernel writes the S2/S3 occupancy map while the state planes pass through it
     FusedArgs args{};
     int npass = 0, pass_nl[2] = { 0, 0 };
@@ -760,8 +761,13 @@ inline int slab_cuts(int ny, int H, short *y0, short *y1, short *o0, short *o1)
 }
 
 template <int NL>
+inline cudaError_t rows_launch(FusedPlan &F, const FusedArgs &A, int grid, cudaStream_t st);   // ca_rows.cuh
+inline bool rows_configure(const KParams &P, FusedPlan &F);
+
+template <int NL>
 inline cudaError_t fused_launch_nl(FusedPlan &F, const FusedArgs &A, int grid, cudaStream_t st)
 {
+    if (F.tiled && F.rows) return rows_launch<NL>(F, A, grid, st);
     if (F.tiled) return fused_launch_slab<NL>(F, A, grid, st);
     if (F.fixed == 64) return fused_launch_t<NL, 32, 64, 64>(F, A, grid, st);
     if (F.fixed == 32) return fused_launch_t<NL, 16, 32, 32>(F, A, grid, st);
@@ -776,7 +782,11 @@ inline void fused_configure(const KParams &P, FusedPlan &F)
     F.tiled = (P.nx > 64 || P.ny > 64);
     if (P.nz < 3 || P.n_sub < 1 || P.n_sub > 2 * F_MAXNL || P.nx < 4) return;
     FusedGeom G{};
-    if (F.tiled) {
+    F.rows = F.tiled && rows_configure(P, F);
+    if (F.rows) {
+        F.fixed = 0;
+        F.writes_map = (P.nx * P.ny) % 256 == 0;
+    } else if (F.tiled) {
         // rows must be whole 16-byte units of the state array (bulk copies) and whole row groups of 2 * LRP sites
         if (P.nx % 16 || P.ny % F_PY) return;
         F.lrp = P.nx % 64 == 0 ? 32 : (P.nx % 32 == 0 ? 16 : 8);

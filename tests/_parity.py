@@ -52,3 +52,32 @@ def assert_fields_bitwise(g, r32, where=""):
         if not np.array_equal(g[k], r32[k].astype(np.float32)):
             bad = np.argwhere(g[k] != r32[k].astype(np.float32))
             raise AssertionError("%s: field %s differs bitwise at %d sites, first %s" % (where, k, len(bad), bad[0]))
+
+
+def assert_close_to_f64_up_to_threshold_flips(g, r, params, n_live, where="", max_frac=5e-4, tol=1e-4, halo=4):
+    """Against the fp64 oracle on a LARGE tumour: a cell whose glucose / H+ / O2 sits within rounding of a mode threshold
+    may take the metabolic-mode decision differently in fp32 and fp64 (the fp32 build of the oracle,
+    which takes every decision in the kernel's precision, must match bit for bit and is checked separately).  Such flips
+    must be rare (<= max_frac of the live cells); away from them (`halo` sites) at most 1 % of the sites may exceed `tol`
+    (traces of flips that have flipped back), none by more than 0.1, and the median error stays at rounding level."""
+    bad = (g["state"] != r["state"]) | (g["clock"] != r["clock"]) | (g["damage"] != r["damage"])
+    nbad = int(bad.sum())
+    assert nbad <= max(2, max_frac * n_live), "%s: %d differing sites of %d live cells" % (where, nbad, n_live)
+    near = bad.copy()
+    for _ in range(halo):
+        grown = near.copy()
+        for ax in range(3):
+            grown |= np.roll(near, 1, ax) | np.roll(near, -1, ax)
+        near = grown
+    for s, k in enumerate(FIELDS):
+        floor = 1e-3 * float(np.float32(params["boundary"][s]))
+        a, b = g[k].astype(np.float64), r[k].astype(np.float64)
+        err = np.abs(a - b) / np.maximum(np.abs(b), floor)
+        err[near] = 0.0
+        # a flip that has flipped back by the end of the window leaves no trace in the state, only in the fields around it (the
+        # anoxic core of a large spheroid sits ON the aerobic threshold and regulates itself there): such sites must stay few
+        # and their error bounded by a few steps' worth of uptake; everywhere else the usual tolerance holds
+        frac = float((err > tol).mean())
+        assert frac <= 0.01 and err.max() <= 0.1, "%s: field %s: %.4f of the sites above %.1e, max rel err %.3e" % (where, k, frac, tol, err.max())
+        assert float(np.median(err)) <= 1e-6, (where, k, float(np.median(err)))
+    return nbad
