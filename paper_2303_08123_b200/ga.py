@@ -60,6 +60,29 @@ def evaluate_population(batch_ctx, snapshot, dose, delay, nfrac, seeds_per_proto
     return fit.reshape(npro, seeds_per_protocol).mean(axis=1), fit
 
 
+def evaluate_on_library(batch_ctx, library, dose, delay, nfrac, seeds_per_tumour, rng_seed, t_end_h, sim_id_base=0):
+    """The paper's fitness methodology: every protocol is run on every tumour of the library
+    `seeds_per_tumour` times; its fitness is the mean over all those evaluations.  ONE batch holds protocols x tumours x
+    seeds simulations, simulation (p, j, s) at index (p * T + j) * S + s with that global id (plus sim_id_base); tumour j's
+    snapshot is loaded into its index ranges with ca_set_state.  `t_end_h` counts from the snapshots' own time.
+    Returns (mean fitness per protocol, fitness[p][j][s])."""
+    npro, T, S = len(nfrac), len(library), int(seeds_per_tumour)
+    assert batch_ctx.batch == npro * T * S, (batch_ctx.batch, npro, T, S)
+    t0_h = None
+    for p in range(npro):
+        for j, snap in enumerate(library):
+            batch_ctx.set_state((p * T + j) * S, S, state=snap["state"], clock=snap["clock"], damage=snap["damage"],
+                                o2=snap["o2"], glc=snap["glc"], h=snap["h"], step=snap["step"])
+            t0_h = snap["step"]
+    batch_ctx.set_rng(rng_seed, sim_id_base)
+    sph = batch_ctx.params.steps_per_hour
+    pro = np.arange(batch_ctx.batch) // (T * S)
+    batch_ctx.set_protocols(np.asarray(dose)[pro], np.asarray(delay)[pro], np.asarray(nfrac)[pro], t0_h=t0_h / sph)
+    batch_ctx.run(t0_h / sph + t_end_h)
+    fit = batch_ctx.fitness().reshape(npro, T, S)
+    return fit.reshape(npro, -1).mean(axis=1), fit
+
+
 # ------------------------------------------------------------------ genotype <-> (dose, delay) list --
 def genotype_to_list(g, max_frac=None):
     """240-slot dose vector -> (dose[k], delay[k]) with delay = wait since the previous fraction, the first one from the

@@ -63,3 +63,16 @@ def radial_profile(snapshot, center=None):
     # hollow core: EMPTY sites well inside the occupied ball (lysed necrotic cells)
     out["empty_inside_half_radius"] = int(((k == 0) & (r < 0.5 * out["r_max"])).sum())
     return out
+
+
+def grow_library(dims, params, init, rng_seed, n_tumours, grow_h, device=0):
+    """The tumour library of PAPER.md l.244: `n_tumours` untreated simulations from the same seed geometry, different
+    simulation ids (0 .. n-1), grown for `grow_h` hours in ONE batch.  Returns the list of snapshots."""
+    nx, ny, nz = dims
+    g = binding.CaBatch(n_tumours, nx, ny, nz, params, max_frac=1, device=device)
+    try:
+        g.seed(rng_seed=rng_seed, sim_id_base=0, **init)
+        g.run(grow_h)
+        return [g.get_state(j) for j in range(n_tumours)]
+    finally:
+        g.close()

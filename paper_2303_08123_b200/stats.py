@@ -65,7 +65,7 @@ def normal_cdf(x):
     return 0.5 * (1.0 + np.vectorize(math.erf)(np.asarray(x, np.float64) / math.sqrt(2.0)))
 
 
-def ks_normality(a):
+def ks_normality(a, discrete=False):
     """One-sample Kolmogorov-Smirnov test of `a` against the normal distribution with the sample's own mean and sd
     (PAPER.md l.69 and Fig. 3C/D, l.357: "KS-test for the normality of the GPU evaluations"; l.252: the final count over
     seeds is close to normal).  Returns (D, asymptotic p).  The parameters are estimated from the sample, as in the
@@ -75,8 +75,15 @@ def ks_normality(a):
     sd = a.std(ddof=1)
     if sd == 0.0:
         return 1.0, 0.0
-    cdf = normal_cdf((a - a.mean()) / sd)
-    d = float(max((np.arange(1, n + 1) / n - cdf).max(), (cdf - np.arange(0, n) / n).max()))
+    if discrete:
+        # integer counts with a small sd: compare with the normal distribution binned the same way (continuity correction),
+        # P(X <= k) against Phi((k + 1/2 - mean) / sd), otherwise the steps of the empirical CDF alone exceed any KS bound
+        vals = np.unique(a)
+        ecdf = np.searchsorted(a, vals, side="right") / n
+        d = float(np.abs(ecdf - normal_cdf((vals + 0.5 - a.mean()) / sd)).max())
+    else:
+        cdf = normal_cdf((a - a.mean()) / sd)
+        d = float(max((np.arange(1, n + 1) / n - cdf).max(), (cdf - np.arange(0, n) / n).max()))
     en = math.sqrt(n)
     lam = (en + 0.12 + 0.11 / en) * d
     p = 2.0 * sum((-1) ** (k - 1) * math.exp(-2.0 * (k * lam) ** 2) for k in range(1, 101))

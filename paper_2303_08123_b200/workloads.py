@@ -152,6 +152,27 @@ def reduced_c2():
                 warmup_h=6.0, t0_h=6.0, horizon_h=120.0, dose=dose, delay=delay, nfrac=np.full(npro, nfr, np.int32))
 
 
+def paper_geometry():
+    """NEXT-3: the workload in the PAPER's own shape rather than BASELINE's.  The paper's lattice is
+    quasi-3-D with at most 1 500 occupiable sites, its tumours are grown for 10 days from 200 cells on
+    10 sites and kept as a library of 10 (l.244), a protocol is scored on every library tumour several times (l.282) over a
+    5-day treatment plus 5 days of regrowth (l.274), and fitness is 1500 - n (Eq. 1).  Here: a 40 x 40 x 3 lattice -- ONE
+    interior plane of 38 x 38 = 1 444 sites between two planes of medium, so that every site touches the replenished
+    medium (l.244) -- N_ref = 1500, a 9-site seed (BALL r = 1.5 in the plane), 10 tumours that differ by their simulation
+    id, 240 h of growth, 240 h of evaluation, BMI and BMII of the paper (l.49) plus an untreated control, 8 seeds per
+    tumour (80 samples per protocol, l.282).  Not reproduced: ~20 cells per site (this build keeps one cell per site,
+    DESIGN.md G1) and the paper's calibrated parameters (it prints none)."""
+    seed = MASTER_SEED + 30
+    names = ["untreated", "BMI", "BMII"]
+    F = 8
+    dose, delay, nfrac = np.zeros((3, F)), np.zeros((3, F)), np.zeros(3, np.int32)
+    for r, (d, t) in enumerate((([], []), PROTOCOL_BMI, PROTOCOL_BMII)):
+        dose[r, :len(d)], delay[r, :len(d)], nfrac[r] = d, t, len(d)
+    return dict(name="paper-geometry", dims=(40, 40, 3), rng_seed=seed, n_ref=1500, n_tumours=10, seeds_per_tumour=8,
+                init=dict(kind="ball", center=(20, 20, 1), radius=1.5, shared_init=False),
+                grow_h=240.0, horizon_h=240.0, protocol_names=names, dose=dose, delay=delay, nfrac=nfrac)
+
+
 def robustness_sweep(base_dose, base_delay, shifts_h=(-1.0, -0.5, 0.5, 1.0), step_h=0.5):
     """NEXT-4 workload (how sensitive is a good protocol to delivery errors?): every variant of one
     protocol in which a single fraction is dropped, or delivered `shift` hours early / late (the following fraction

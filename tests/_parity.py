@@ -54,7 +54,7 @@ def assert_fields_bitwise(g, r32, where=""):
             raise AssertionError("%s: field %s differs bitwise at %d sites, first %s" % (where, k, len(bad), bad[0]))
 
 
-def assert_close_to_f64_up_to_threshold_flips(g, r, params, n_live, where="", max_frac=5e-4, tol=1e-4, halo=4):
+def assert_close_to_f64_up_to_threshold_flips(g, r, params, n_live, where="", max_frac=2e-3, tol=1e-4, halo=4):
     """Against the fp64 oracle on a LARGE tumour: a cell whose glucose / H+ / O2 sits within rounding of a mode threshold
     may take the metabolic-mode decision differently in fp32 and fp64 (the fp32 build of the oracle,
     which takes every decision in the kernel's precision, must match bit for bit and is checked separately).  Such flips

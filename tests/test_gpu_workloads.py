@@ -137,13 +137,12 @@ def test_next2_final_count_over_2000_seeds_is_close_to_normal():
     g.run(cfg["horizon_h"])
     cnt = g.counts()
     occ = cnt[:, 12].astype(np.float64)
-    d, pval = stats.ks_normality(occ)
+    d, pval = stats.ks_normality(occ, discrete=True)              # integer counts, sd of a few cells: binned comparison
     mean, sd = occ.mean(), occ.std(ddof=1)
     assert sd > 0 and 0.02 < sd / mean < 0.5, (mean, sd)
-    # integer counts with sd ~ 10 make the KS statistic of a truly normal variable a little larger than in the continuum
-    assert d < 0.05 and pval > 1e-3, (d, pval, mean, sd)
+    assert d < 0.04 and pval > 1e-3, (d, pval, mean, sd)
     skew = float(((occ - mean) ** 3).mean() / sd ** 3)
-    assert abs(skew) < 0.5, skew
+    assert abs(skew) < 0.6, skew
     r = o.OracleSim(*cfg["dims"], p, precision="f32")
     r.seed(cfg["init"]["kind"], center=cfg["init"]["center"], rng_seed=cfg["rng_seed"], sim_id=0)
     r.set_protocol(cfg["dose"][0], cfg["delay"][0], t0_h=cfg["t0_h"])
@@ -189,3 +188,37 @@ def test_long_horizon_statistical_parity_with_the_fp64_oracle_ensemble():
     # the trajectories share their random streams: most simulations still agree exactly with the fp64 oracle after 75 600 steps
     same = float((gpu_occ == ref_occ).mean())
     assert same > 0.5, same
+
+
+def test_next3_paper_geometry_library_fitness_methodology_and_whole_run_parity():
+    """NEXT-3: the paper-shaped workload -- one-plane lattice of <= 1500 sites, a library
+    of 10 tumours grown for 10 days from a ~10-site seed, every protocol scored on every tumour x 8 seeds over 5 days of
+    treatment + 5 days of regrowth, fitness = 1500 - n (Eq. 1), ITS against the untreated control (Eq. 2).  One of the 240
+    simulations is re-run WHOLE (144 000 steps) by the fp32 build of the oracle from the same library snapshot: same counts."""
+    from paper_2303_08123_b200 import ga
+    cfg = w.paper_geometry()
+    p = w.default_params(N_ref=cfg["n_ref"])
+    dims = cfg["dims"]
+    lib = pregrow.grow_library(dims, p, cfg["init"], cfg["rng_seed"], cfg["n_tumours"], cfg["grow_h"])
+    occ0 = np.array([int((((s["state"] & 7) >= 1) & ((s["state"] & 7) <= 5)).sum()) for s in lib])
+    assert len(set(occ0.tolist())) > 3 and occ0.min() > 60 and occ0.max() < 1200, occ0       # ten different tumours that fit the plane
+    T, S, npro = cfg["n_tumours"], cfg["seeds_per_tumour"], len(cfg["nfrac"])
+    g = binding.CaBatch(npro * T * S, *dims, p, max_frac=cfg["dose"].shape[1])
+    mean_fit, fit = ga.evaluate_on_library(g, lib, cfg["dose"], cfg["delay"], cfg["nfrac"], S, cfg["rng_seed"], cfg["horizon_h"])
+    cnt = g.counts()
+    assert fit.shape == (npro, T, S) and g.step_index == int(round((cfg["grow_h"] + cfg["horizon_h"]) * 600))
+    n_mean = stats.occupied_from_fitness(mean_fit, cfg["n_ref"])
+    assert (fit <= 1500).all() and (fit >= 1500 - 38 * 38).all()
+    assert n_mean[0] > n_mean[1] and n_mean[0] > n_mean[2], n_mean                              # both benchmarks beat no treatment
+    assert stats.its(n_mean[1], n_mean[0]) > 0.02 and stats.its(n_mean[2], n_mean[0]) > 0.02
+    sd = fit.reshape(npro, -1).std(axis=1, ddof=1)
+    assert (sd > 0).all()
+    # whole-run parity of one simulation (BMII, tumour 3, seed 5)
+    pr, j, s = 2, 3, 5
+    b = (pr * T + j) * S + s
+    r = oracle_from_snapshot(lib[j], p, dims, cfg["rng_seed"], b, precision="f32")
+    r.set_protocol(cfg["dose"][pr][:cfg["nfrac"][pr]], cfg["delay"][pr][:cfg["nfrac"][pr]], t0_h=cfg["grow_h"])
+    r.run(cfg["grow_h"] + cfg["horizon_h"])
+    assert cnt[b].tolist() == r.counts().tolist()
+    assert fit[pr, j, s] == r.fitness()
+    g.close()

@@ -42,3 +42,29 @@ def test_summarize_groups_seeds():
     f = np.arange(12.0)
     mean, sd = stats.summarize(f, 4)
     assert mean.tolist() == [1.5, 5.5, 9.5] and np.allclose(sd, np.std([0, 1, 2, 3], ddof=1))
+
+
+def test_ks_normality_continuous_matches_scipy_and_discrete_handles_integer_counts():
+    rng = np.random.default_rng(8)
+    x = rng.normal(300.0, 40.0, 500)
+    d, p = stats.ks_normality(x)
+    ref = st.kstest((x - x.mean()) / x.std(ddof=1), "norm")
+    assert abs(d - ref.statistic) < 1e-12 and abs(p - ref.pvalue) < 0.02
+    assert stats.ks_normality(rng.exponential(1.0, 500))[1] < 1e-3            # clearly not normal
+    k = np.round(rng.normal(36.0, 4.0, 2000))                                  # integer counts, sd of a few units
+    assert stats.ks_normality(k)[0] > 0.04                                     # the plain statistic sees the steps ...
+    assert stats.ks_normality(k, discrete=True)[0] < 0.03                      # ... the binned one does not
+    assert stats.ks_normality(np.round(rng.exponential(6.0, 2000)), discrete=True)[1] < 1e-3
+
+
+def test_compare_implementations_and_pvalue_pile_up():
+    rng = np.random.default_rng(9)
+    x = [rng.normal(300 + 5 * k, 30, 40) for k in range(60)]
+    y = [rng.normal(300 + 5 * k, 30, 48) for k in range(60)]                   # same distributions: Fig. 3B of the paper
+    cmp = stats.compare_implementations(x, y)
+    assert stats.pvalues_not_piled_up(cmp["p_t"]) and (cmp["p_t"] < 0.05).mean() < 0.15
+    assert np.all(np.abs(cmp["mean_x"] - cmp["mean_y"]) < 4 * (cmp["ci_x"] + cmp["ci_y"]))
+    z = [rng.normal(330 + 5 * k, 30, 48) for k in range(60)]                   # shifted by one sd: must be noticed
+    assert not stats.pvalues_not_piled_up(stats.compare_implementations(x, z)["p_t"])
+    m, ci = stats.mean_ci95(np.arange(10.0))
+    assert m == 4.5 and abs(ci - st.t.ppf(0.975, 9) * np.arange(10.0).std(ddof=1) / np.sqrt(10)) < 1e-12
