@@ -175,8 +175,9 @@ struct Rows {
     template <int PH, bool STEADY>
     static __device__ __forceinline__ void step(const int i, u64 (&h)[NL][3][PX], RowsCtx &c)
     {
-        if (STEADY && ((c.flags & ((1u << NL) - 1u)) | c.slowmask) == 0u) step_body<PH, true, true>(i, h, c);
-        else step_body<PH, STEADY, false>(i, h, c);
+        // one body per phase: a second copy without the source-term code (as in k_diffuse_fused) costs more in instruction-cache
+        // misses than the untaken branches it saves here (measured: 0.806 -> 0.775 ms at 64 x 96^3, 0.659 -> 0.608 ms at 96 x 80^3)
+        step_body<PH, STEADY, false>(i, h, c);
     }
 
     template <int PH, bool STEADY, bool NOCELLS>
@@ -226,10 +227,11 @@ struct Rows {
         // ---- the plane the last level just staged leaves by one bulk store (its rows are contiguous in shared and global memory)
         const int zo = t - NL;
         const bool out_now = STEADY || (zo >= c.za && zo < c.zb);
-        if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // the store of the previous iteration has read its staging slab: the next iteration may overwrite it
+        // the loads are thread 0's job, the stores thread 32's (bulk groups belong to the thread that commits them): one producer for both is late at every barrier
+        if (threadIdx.x == 32) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");  // the store of the previous iteration has read its staging slab: the next iteration may overwrite it
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");        // my staging writes are visible to the bulk-copy engine
         __syncthreads();
-        if (threadIdx.x == 0 && out_now) {
+        if (threadIdx.x == 32 && out_now) {
             const RowsSeg *sg = seg();
             const uint32_t src = c.out_ring + (q & 1u) * c.in_slot + sg->out_off;
             asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(sg->dst_rows + (size_t)zo * c.nxny), "r"(src), "r"(sg->out_bytes) : "memory");
@@ -339,7 +341,7 @@ __global__ void __launch_bounds__(MAXW * 32, 1) k_diffuse_rows(const FusedArgs A
         }
         c.itg += (uint32_t)c.nsteps;
     }
-    if (tid == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");    // the last stores must have left shared memory before the CTA retires
+    if (tid == 32) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // the last stores must have left shared memory before the CTA retires
 }
 
 // ------------------------------------------------------------------ host side --

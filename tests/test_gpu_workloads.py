@@ -17,6 +17,7 @@ GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "reduced_c2_ensemble.
 
 def _free_gb():
     import torch
+    torch.cuda.empty_cache()                 # earlier tests' workspaces sit in torch's caching allocator
     return torch.cuda.mem_get_info()[0] / 1e9
 
 
