@@ -280,12 +280,14 @@ def timed_window(torch, g, stream, t_start, dt_h, warmup, steps, fit_dev):
     return e0.elapsed_time(e1), t
 
 
-def config_probe(torch, binding, name, cfg, params, snap, device, ca_steps, kernel, traffic_pattern):
+def config_probe(torch, binding, name, cfg, params, snap, device, ca_steps, kernel, traffic_pattern, options=None):
     """one per_config entry: the whole CA step and its diffusion kernel on this configuration, measured now"""
     B = cfg["batch"]
     nx, ny, nz = cfg["dims"]
     sites = nx * ny * nz
     g = binding.CaBatch(B, nx, ny, nz, params, max_frac=cfg["dose"].shape[1], device=device)
+    for k, v in (options or {}).items():
+        g.set_option(k, v)
     load_snapshot(g, snap)
     g.set_rng(cfg["rng_seed"], 0)
     g.set_protocols(cfg["dose"], cfg["delay"], cfg["nfrac"], t0_h=cfg["t0_h"])
@@ -295,6 +297,10 @@ def config_probe(torch, binding, name, cfg, params, snap, device, ca_steps, kern
     step_ms = ms / 3 / ca_steps
     stage_ms, nl = time_stage(torch, g, g.stream, 10)
     cnt = g.counts()
+    kern = {0: "k_diffuse_sub", 1: "k_diffuse_fused", 2: "k_diffuse_slab", 3: "k_diffuse_rows"}[g.get_option("diffusion_kernel")]
+    if g.get_option("rows_cluster"):
+        kern += " (clusters of %d CTAs, %d resident)" % (g.get_option("rows_cluster"), g.get_option("rows_nclusters"))
+    kernel = kern
     out = {"workload": "BASELINE configs[%s]: %d sims x %dx%dx%d" % (name, B, nx, ny, nz), "batch": B, "dims": [nx, ny, nz],
            "resident_gb": 29.0 * B * sites / 1e9, "ca_steps_timed": 3 * ca_steps, "us_per_ca_step": step_ms * 1e3,
            "site_updates_per_s": B * sites / (step_ms * 1e-3), "live_cells_per_sim_mean": float(cnt[:, 0].mean()),
@@ -430,7 +436,8 @@ def run_probe(args):
             cfg["init"] = dict(cfg["init"], kind="ball", radius=float(args.tumour_radius))
         snap = warm_snapshot(binding, cfg, params, 0)
     kern = "k_diffuse_fused" if k == 2 else "k_diffuse_rows"
-    out = config_probe(torch, binding, str(k - 1), cfg, params, snap, 0, args.ca_steps or (200 if k == 2 else 20), kern, None)
+    opts = {} if args.rows_cluster is None else {"rows_cluster": args.rows_cluster}
+    out = config_probe(torch, binding, str(k - 1), cfg, params, snap, 0, args.ca_steps or (200 if k == 2 else 20), kern, None, options=opts)
     out["probe"] = {"config": args.probe, "batch": cfg["batch"], "tumour_radius": args.tumour_radius}
     print(json.dumps(out))
 
@@ -618,6 +625,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--probe", default=None, choices=["c2", "c3", "c4"], help="measure ONE configuration alone (with --batch: reduced batch) and print its per_config entry")
     ap.add_argument("--tumour-radius", type=float, default=None, help="--probe only: start from a seeded BALL of this radius (late, dense phase)")
+    ap.add_argument("--rows-cluster", type=int, default=None, help="--probe c3 only: 0 = slabs with a halo, 3 = clusters of 3 CTAs per plane")
     ap.add_argument("--ga", action="store_true", help="configs[4] sharded population evaluation + host GA loop at reduced size")
     ap.add_argument("--ga-population", type=int, default=128)
     ap.add_argument("--ga-generations", type=int, default=2)

@@ -160,9 +160,14 @@ int ca_stage(ca_ctx *c, int stage, int arg);
  *   "fused"        1 = temporally fused diffusion kernels (default), 0 = one launch per sub-step
  *   "cell_path"    1 = clustered S2+S3 kernel driven by the occupancy map when the lattice allows (default), 0 = generic scans
  *   "cluster"      CTAs per simulation of the clustered kernel: 1, 2, 4 or 8
+ *   "rows_cluster" 3 = k_diffuse_rows as clusters of 3 CTAs per 96 x 96 plane (boundary rows through distributed shared
+ *                  memory, no halo), 0 = y-slabs with a halo
  *   "inject_launch_error"  1 = fault injection: the next step / stage call behaves as if a kernel launch had failed
  * CA_EINVAL on an unknown name or value. */
 int ca_set_option(ca_ctx *c, const char *name, int value);
+/* Read a knob back (HOST out), plus: "diffusion_kernel" (0 k_diffuse_sub, 1 k_diffuse_fused, 2 k_diffuse_slab,
+ * 3 k_diffuse_rows: which kernel runs S1 on this lattice), "rows_cluster", "rows_nclusters". */
+int ca_get_option(ca_ctx *c, const char *name, int *value);
 /* Number of kernel launches (graph nodes included) issued by this context so far. */
 int64_t ca_launch_count(ca_ctx *c);
 

@@ -19,7 +19,7 @@ INIT_KINDS = {"single": 0, "cluster7": 1, "ball": 2}
 
 EXPORTS = ("ca_version", "ca_last_error", "ca_workspace_bytes", "ca_create", "ca_destroy", "ca_seed", "ca_set_rng",
            "ca_set_protocols", "ca_run", "ca_step", "ca_get_step", "ca_sync", "ca_fitness", "ca_counts",
-           "ca_get_state", "ca_set_state", "ca_stage", "ca_set_option", "ca_launch_count")
+           "ca_get_state", "ca_set_state", "ca_stage", "ca_set_option", "ca_get_option", "ca_launch_count")
 
 
 class CaParams(C.Structure):
@@ -81,6 +81,7 @@ def load():
     L.ca_set_state.argtypes = [vp, C.c_int, C.c_int, vp, vp, vp, vp, vp, vp, C.c_int64]
     L.ca_stage.argtypes = [vp, C.c_int, C.c_int]
     L.ca_set_option.argtypes = [vp, C.c_char_p, C.c_int]
+    L.ca_get_option.argtypes = [vp, C.c_char_p, C.POINTER(C.c_int)]
     L.ca_launch_count.argtypes = [vp]
     L.ca_launch_count.restype = C.c_int64
     _LIB = L
@@ -228,6 +229,11 @@ class CaBatch:
 
     def set_option(self, name, value):
         self._chk(self.L.ca_set_option(self.ctx, name.encode(), int(value)))
+
+    def get_option(self, name):
+        v = C.c_int()
+        self._chk(self.L.ca_get_option(self.ctx, name.encode(), C.byref(v)))
+        return int(v.value)
 
     @property
     def launch_count(self):

@@ -665,6 +665,10 @@ int ca_set_option(ca_ctx *c, const char *name, int value)
     if (!std::strcmp(name, "inject_launch_error")) {                          // fault injection for the tests: the next step sees a failed kernel launch
         c->launch_err = value ? cudaErrorLaunchOutOfResources : cudaSuccess; return CA_OK;
     }
+    if (!std::strcmp(name, "rows_cluster")) {                                  // 0: k_diffuse_rows on slabs with a halo; 3: cluster of 3 CTAs per 96 x 96 plane
+        if (!(value == 0 || (value == 3 && c->P.nx == 96 && c->P.ny == 96 && c->fplan.rows))) return fail(c, CA_EINVAL, "rows_cluster must be 0, or 3 on 96 x 96 planes");
+        c->fplan.rows_cluster = value; drop_graphs(c); return CA_OK;
+    }
     if (!std::strcmp(name, "cluster")) {
         if (value != 1 && value != 2 && value != 4 && value != 8) return fail(c, CA_EINVAL, "cluster must be 1, 2, 4 or 8");
         c->cs = value; drop_graphs(c); return CA_OK;
@@ -672,6 +676,22 @@ int ca_set_option(ca_ctx *c, const char *name, int value)
     if (!std::strcmp(name, "cell_path")) {
         c->cell_path = value ? 1 : 0; drop_graphs(c);
         cudaMemsetAsync(c->d_lys, 1, (size_t)c->P.batch * 4, c->stream);     // the generic path does not track lysis: re-evaluate every parent once
+        return CA_OK;
+    }
+    return fail(c, CA_EINVAL, std::string("unknown option ") + name);
+}
+
+int ca_get_option(ca_ctx *c, const char *name, int *value)
+{
+    if (!c || !name || !value) return CA_EINVAL;
+    if (!std::strcmp(name, "graph_steps")) { *value = c->graph_steps; return CA_OK; }
+    if (!std::strcmp(name, "fused")) { *value = c->fused && fused_supported(c->fplan); return CA_OK; }
+    if (!std::strcmp(name, "cell_path")) { *value = c->cell_path && c->mapped_ok; return CA_OK; }
+    if (!std::strcmp(name, "cluster")) { *value = c->cs; return CA_OK; }
+    if (!std::strcmp(name, "rows_cluster")) { *value = c->fplan.rows ? c->fplan.rows_cluster : 0; return CA_OK; }
+    if (!std::strcmp(name, "rows_nclusters")) { *value = c->fplan.nclusters; return CA_OK; }   // resident clusters of the last cluster launch (0 before it)
+    if (!std::strcmp(name, "diffusion_kernel")) {                             // 0 k_diffuse_sub, 1 k_diffuse_fused, 2 k_diffuse_slab, 3 k_diffuse_rows
+        *value = !(c->fused && fused_supported(c->fplan)) ? 0 : (!c->fplan.tiled ? 1 : (c->fplan.rows ? 3 : 2));
         return CA_OK;
     }
     return fail(c, CA_EINVAL, std::string("unknown option ") + name);

@@ -54,9 +54,29 @@ struct RowsCtx {
     u64 lamL, lamM, lamR;          // lambda pairs (row 0, row 1) for the lane's first / middle / last column; WALL and frozen rows folded in
     u64 zero2;
     uint32_t occ_nw;               // species 0: occupancy words of a plane this slab writes (else 0)
+    // cluster variant: the CTA's first / last row pair also publishes its outer row into the neighbour CTA's exchange
+    uint32_t rem;                  // shared::cluster address of that row's slot (buffer 0, level 0) in the neighbour's exchange; 0: none
+    bool rem_row1;                 // the row to send: row 1 of the pair (last pair, to the CTA below) or row 0 (first pair, to the CTA above)
 };
 
-template <int NL, int PX, int LRP>
+// cluster helpers (sm_90+): rank inside the cluster, address of a peer CTA's shared memory, cluster-wide barrier
+__device__ __forceinline__ uint32_t cluster_rank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ uint32_t map_to_rank(uint32_t addr, uint32_t rank)
+{
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void st_cluster_f32(uint32_t addr, float v) { asm volatile("st.shared::cluster.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory"); }
+__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_barrier()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+
+// CS = 1: y-slabs with a halo (any ny);  CS > 1: a thread-block cluster of CS CTAs holds ny = CS * hrows rows exactly, no halo
+template <int NL, int PX, int LRP, int CS = 1>
 struct Rows {
     static constexpr int NX = PX * LRP;
     static constexpr int RW = 32 / LRP;                                   // row pairs per warp
@@ -123,6 +143,9 @@ struct Rows {
                                                   u64 (&h)[NL][3][PX], RowsCtx &c)
     {
         if constexpr (K <= NL) {
+            // cluster variant: every row the neighbours need from this iteration is published once level NL-1 is done; the last
+            // level (a quarter of the arithmetic, staging only) runs between the arrive and the wait at the top of the next iteration
+            if constexpr (CS > 1 && K == NL) cluster_arrive();
             constexpr int sm = (PH - K - 1 + 12) % 3, sc = (PH - K + 12) % 3, sp = (PH - K + 1 + 12) % 3;
             constexpr int KO = K < NL ? K : 0;
             const int zc = t - K;
@@ -162,6 +185,17 @@ struct Rows {
                     asm volatile("st.shared.f32 [%0], %1;" ::"r"(wb + (uint32_t)k * 4u), "f"(a) : "memory");
                     asm volatile("st.shared.f32 [%0], %1;" ::"r"(wb + PITCH + (uint32_t)k * 4u), "f"(b) : "memory");
                 }
+                if constexpr (CS > 1 && K < NL) {                            // my outer row is the neighbour CTA's halo row of level K
+                    if (c.rem != 0u) {
+                        const uint32_t ra = c.rem + (exw - c.ex_lane) + (uint32_t)K * c.ex_lvl;
+#pragma unroll
+                        for (int k = 0; k < PX; ++k) {
+                            float a, b;
+                            upk(N[k], a, b);
+                            st_cluster_f32(ra + (uint32_t)k * 4u, c.rem_row1 ? b : a);
+                        }
+                    }
+                }
             } else if (K < NL && (zc == 0 || zc == c.nz - 1) && zc >= c.za - (NL - K) && zc < c.zb + (NL - K)) {
                 // WALL plane: every level equals the input there
                 const float *p = c.src + (size_t)zc * c.nxny;
@@ -190,6 +224,7 @@ struct Rows {
         const uint32_t exw = c.ex_lane + ((uint32_t)i & 1u) * exb;           // rows written now, read by the next iteration
         const uint32_t exr = c.ex_lane + exb - ((uint32_t)i & 1u) * exb;     // rows written by the previous iteration
         const uint32_t outw = c.out_ring + (q & 1u) * c.in_slot + c.lane_b;
+        if constexpr (CS > 1) cluster_wait();                                // the neighbours' rows of the previous iteration have arrived, and they have read mine
         // ---- level 0: plane t from the ring
         mbar_wait(c.bars + 8u * PH, (c.par >> PH) & 1u);
         c.par ^= 1u << PH;
@@ -202,6 +237,9 @@ struct Rows {
                 h[0][PH][k] = pk(v0, v1);
                 asm volatile("st.shared.f32 [%0], %1;" ::"r"(exw + PITCH + (uint32_t)k * 4u), "f"(v0) : "memory");
                 asm volatile("st.shared.f32 [%0], %1;" ::"r"(exw + 2u * PITCH + (uint32_t)k * 4u), "f"(v1) : "memory");
+                if constexpr (CS > 1) {
+                    if (c.rem != 0u) st_cluster_f32(c.rem + (exw - c.ex_lane) + (uint32_t)k * 4u, c.rem_row1 ? v1 : v0);
+                }
             }
             const uint32_t sbase = c.st_ring + (q & (F_SRING - 1)) * c.st_slot;
             // "cells in my warp's rows": the warp's rows are contiguous bytes of the state slab; a byte counts when kind is 1..6
@@ -241,10 +279,10 @@ struct Rows {
 };
 
 // grid: persistent, one CTA per SM; block = Gm.nwarps warps
-template <int NL, int PX, int LRP, int MAXW>
+template <int NL, int PX, int LRP, int MAXW, int CS>
 __global__ void __launch_bounds__(MAXW * 32, 1) k_diffuse_rows(const FusedArgs A, const RowsGeom Gm)
 {
-    typedef Rows<NL, PX, LRP> R;
+    typedef Rows<NL, PX, LRP, CS> R;
     extern __shared__ __align__(128) unsigned char rsm[];
     constexpr int NX = PX * LRP, RW = 32 / LRP;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -266,11 +304,23 @@ __global__ void __launch_bounds__(MAXW * 32, 1) k_diffuse_rows(const FusedArgs A
     }
     for (int e = tid; e < 96; e += blockDim.x) reinterpret_cast<float *>(rsm + Gm.off_lut)[e] = A.lut[e / 32][e % 32];
     for (uint32_t e = tid; e < (Gm.smem_bytes - Gm.off_ex) / 8u; e += blockDim.x) reinterpret_cast<u64 *>(rsm + Gm.off_ex)[e] = 0ull;   // exchange and staging
-    __syncthreads();
+    const int rank = CS > 1 ? (int)cluster_rank() : 0;
+    c.rem = 0u; c.rem_row1 = false;
+    if constexpr (CS > 1) {
+        // the CTAs of a cluster hold consecutive ranges of hrows rows; exchange row 0 / hrows + 1 of a CTA is written by its neighbour
+        const int pairs = Gm.hrows / 2;
+        if (gl == 0 && rank > 0) c.rem = map_to_rank(base + Gm.off_ex + (uint32_t)(Gm.hrows + 1) * R::PITCH + (uint32_t)x0 * 4u, (uint32_t)(rank - 1));
+        if (gl == pairs - 1 && rank < CS - 1) { c.rem = map_to_rank(base + Gm.off_ex + (uint32_t)x0 * 4u, (uint32_t)(rank + 1)); c.rem_row1 = true; }
+        cluster_barrier();                                                   // nobody writes into an exchange that is still being zeroed
+        cluster_arrive();                                                    // pairs with the wait at the top of the first iteration
+    } else {
+        __syncthreads();
+    }
 
     const int nzi = A.nz - 2;
-    long long p = Gm.start[blockIdx.x];
-    const long long p_end = Gm.start[blockIdx.x + 1];
+    const int wid = CS > 1 ? (int)blockIdx.x / CS : (int)blockIdx.x;       // the CTAs of a cluster work through the same segments in lockstep
+    long long p = Gm.start[wid];
+    const long long p_end = Gm.start[wid + 1];
     u64 h[NL][3][PX];
 #pragma unroll
     for (int k = 0; k < NL; ++k)
@@ -281,7 +331,7 @@ __global__ void __launch_bounds__(MAXW * 32, 1) k_diffuse_rows(const FusedArgs A
 
     while (p < p_end) {
         const int unit = (int)(p / nzi);
-        const int slab = unit % A.nslab, us = unit / A.nslab;
+        const int slab = CS > 1 ? rank : unit % A.nslab, us = CS > 1 ? unit : unit / A.nslab;
         const int b = us / 3, sp = us % 3;
         c.za = 1 + (int)(p - (long long)unit * nzi);
         c.zb = (int)min((long long)(A.nz - 1), (long long)c.za + (p_end - p));
@@ -307,7 +357,9 @@ __global__ void __launch_bounds__(MAXW * 32, 1) k_diffuse_rows(const FusedArgs A
         if (sp == 0 && A.occ != nullptr) c.occ_nw = (uint32_t)((oy1 * NX + 255) / 256) - (uint32_t)((oy0 * NX + 255) / 256);
         {
             const float l = A.lam[sp];
-            const float m0 = row0 > 0 ? 1.0f : 0.0f, m1 = row0 + 1 < rows - 1 ? 1.0f : 0.0f;   // the slab's first / last row is frozen (WALL, or halo edge)
+            // the slab's first / last row is frozen (WALL, or halo edge); in a cluster only the lattice's own first / last row (WALL)
+            const float m0 = (CS > 1 ? ty0 + row0 > 0 : row0 > 0) ? 1.0f : 0.0f;
+            const float m1 = (CS > 1 ? ty0 + row0 + 1 < A.ny - 1 : row0 + 1 < rows - 1) ? 1.0f : 0.0f;
             c.lamM = pk(l * m0, l * m1);
             c.lamL = lx == 0 ? pk(0.0f, 0.0f) : c.lamM;                        // x = 0 and x = nx-1 are WALL
             c.lamR = lx == LRP - 1 ? pk(0.0f, 0.0f) : c.lamM;
@@ -342,6 +394,7 @@ __global__ void __launch_bounds__(MAXW * 32, 1) k_diffuse_rows(const FusedArgs A
         c.itg += (uint32_t)c.nsteps;
     }
     if (tid == 32) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // the last stores must have left shared memory before the CTA retires
+    if constexpr (CS > 1) { cluster_wait(); cluster_barrier(); }              // the last arrive; and no neighbour may still be sending into a CTA that has gone
 }
 
 // ------------------------------------------------------------------ host side --
@@ -376,18 +429,60 @@ inline cudaError_t rows_launch_t(FusedPlan &F, const FusedArgs &A, int grid, cud
     if (grid > F_MAXGRID) grid = F_MAXGRID;
     fused_split_cached(F, units, A.nz - 2, NL, grid, G.start);
     if (!F.attr_done[NL]) {
-        cudaError_t e = cudaFuncSetAttribute(k_diffuse_rows<NL, PX, LRP, MAXW>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        cudaError_t e = cudaFuncSetAttribute(k_diffuse_rows<NL, PX, LRP, MAXW, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         if (e != cudaSuccess) return e;
         F.attr_done[NL] = true;
     }
-    k_diffuse_rows<NL, PX, LRP, MAXW><<<grid, G.nwarps * 32, G.smem_bytes, st>>>(A, G);
+    k_diffuse_rows<NL, PX, LRP, MAXW, 1><<<grid, G.nwarps * 32, G.smem_bytes, st>>>(A, G);
     return cudaGetLastError();
+}
+
+// Cluster variant: CS CTAs share a plane (ny = CS * hrows exactly), boundary rows travel through distributed shared memory.
+// One cluster per CS SMs, persistent; the (unit, plane) space is split over the clusters.
+template <int NL, int PX, int LRP, int MAXW, int CS>
+inline cudaError_t rows_launch_cluster_t(FusedPlan &F, const FusedArgs &A0, cudaStream_t st)
+{
+    FusedArgs A = A0;
+    const int hrows = A.ny / CS;
+    A.nslab = 1; A.rga = hrows;
+    for (int r = 0; r < CS; ++r) { A.sy0[r] = A.so0[r] = (short)(r * hrows); A.sy1[r] = A.so1[r] = (short)((r + 1) * hrows); }
+    RowsGeom G{};
+    rows_smem(A.nx, NL, hrows, G);
+    G.nwarps = (hrows / 2) / (32 / LRP);
+    auto kern = k_diffuse_rows<NL, PX, LRP, MAXW, CS>;
+    cudaLaunchConfig_t cfg = {};
+    cfg.blockDim = dim3((unsigned int)(G.nwarps * 32));
+    cfg.dynamicSmemBytes = G.smem_bytes;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = CS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    if (!F.cluster_attr_done[NL]) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        if (e != cudaSuccess) return e;
+        if (CS > 8) { e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1); if (e != cudaSuccess) return e; }
+        cfg.gridDim = dim3((unsigned int)(F.sms / CS * CS));
+        int nc = 0;
+        e = cudaOccupancyMaxActiveClusters(&nc, kern, &cfg);
+        if (e != cudaSuccess) return e;
+        if (nc < 1) return cudaErrorLaunchOutOfResources;
+        F.nclusters = nc;
+        F.cluster_attr_done[NL] = true;
+    }
+    const int units = A.batch * 3;
+    const long long total = (long long)units * (A.nz - 2);
+    int ncl = (int)std::max<long long>(1, std::min<long long>(std::min(F.nclusters, F_MAXGRID / CS), total / 2 + 1));
+    fused_split_cached(F, units, A.nz - 2, NL, ncl, G.start);
+    cfg.gridDim = dim3((unsigned int)(ncl * CS));
+    return cudaLaunchKernelEx(&cfg, kern, A, G);
 }
 
 template <int NL>
 inline cudaError_t rows_launch(FusedPlan &F, const FusedArgs &A, int grid, cudaStream_t st)
 {
-    if (A.nx == 96) return rows_launch_t<NL, 3, 32, 16>(F, A, grid, st);      // BASELINE configs[2]
+    if (A.nx == 96 && F.rows_cluster == 3) return rows_launch_cluster_t<NL, 3, 32, 16, 3>(F, A, st);   // BASELINE configs[2]: 3 CTAs x 32 rows
+    if (A.nx == 96) return rows_launch_t<NL, 3, 32, 16>(F, A, grid, st);      // 96-wide planes of any height: slabs with a halo
     return rows_launch_t<NL, 5, 16, 12>(F, A, grid, st);                      // BASELINE configs[3]
 }
 
@@ -406,6 +501,10 @@ inline bool rows_configure(const KParams &P, FusedPlan &F)
     RowsGeom G{};
     if (rows_smem(P.nx, F_MAXNL, hrows, G) > 227 * 1024) return false;
     F.lrp = lrp;
+    // The cluster variant (96 rows = 3 CTAs x 16 warps x one row pair, no halo) is correct and selectable ("rows_cluster" = 3) but
+    // OFF by default: measured 0.851 ms against 0.769 ms for the slabs with a halo at 64 x 96^3 (45 clusters = 135 of 148 SMs
+    // resident, and an iteration of three SMs in lockstep costs 4075 cycles against 3063), DESIGN.md section 7.
+    F.rows_cluster = 0;
     return true;
 }
 

@@ -226,9 +226,10 @@ def test_state_roundtrip_broadcast_and_errors():
     ((32, 32, 12), 6, {"graph_steps": 4}),                   # 3 + 3 levels, two passes (buffer flips twice per step)
     ((32, 32, 12), 5, {"graph_steps": 2}),                   # 3 + 2: odd number of flips per step
     ((48, 32, 9), 2, {}),                                    # run-time-dims fused kernel, map built by k_occ_map
-    ((96, 96, 9), 4, {}),                                    # configs[2] plane: 2 x 2 tiles of 52 x 52 (tiled kernel), spheroid on the tile cut
-    ((80, 80, 9), 4, {"graph_steps": 6}),                    # configs[3] plane: 2 x 2 tiles of 44 x 44
-    ((128, 72, 8), 3, {}),                                   # 3 x 2 tiles of unequal size
+    ((96, 96, 9), 4, {}),                                    # configs[2] plane: k_diffuse_rows, 4 y-slabs of 32 rows, spheroid on the cuts
+    ((96, 96, 9), 4, {"rows_cluster": 3, "graph_steps": 4}), # the same plane on clusters of 3 CTAs: boundary rows through distributed shared memory
+    ((80, 80, 9), 4, {"graph_steps": 6}),                    # configs[3] plane: k_diffuse_rows, 2 y-slabs of 44 rows
+    ((128, 72, 8), 3, {}),                                   # k_diffuse_slab: 2 column blocks with an x-seam, 3 y-slabs
 ])
 def test_fast_path_variants_against_the_oracle(dims, n_sub, opts):
     """Every launch configuration of the fast path gives the oracle's lattice: bit-exact integers and (against the
