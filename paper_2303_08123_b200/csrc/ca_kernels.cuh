@@ -400,12 +400,15 @@ constexpr int CD_WCAP = 2048;     // map words examined per round
 constexpr int CD_TILE = 16;       // map words per interleave tile (one 64x64 plane): CTA rank takes tiles rank, rank + cs, ...
 constexpr int CD_WINCAP = 2048;   // winners per CTA and step
 constexpr int CD_PCAP = 1024;     // READY parents remembered from S2 (more: S3 rescans the map)
+constexpr int CD_GWORDS = 128;    // map words whose set bits are expanded into the group list at a time (128 x 32 bits fill it exactly)
+constexpr int CD_GCAP = CD_GWORDS * 32;
 
 struct CDShared {
     uint32_t W[CD_WCAP];          // indices of the non-empty map words of this round
     uint32_t win[CD_WINCAP];      // winners: parent site << 3 | direction
     uint32_t Pl[CD_PCAP];         // READY parents after S2 (site index inside the simulation)
-    uint32_t nW, nwin, nP;
+    uint32_t G[CD_GCAP];          // occupied groups of 8 sites of the current chunk of map words: word << 5 | bit
+    uint32_t nW, nwin, nP, nG;
 };
 
 __device__ __forceinline__ void cluster_sync_all()
@@ -432,9 +435,11 @@ __device__ __forceinline__ void cd_winner(CDShared &sh, uint32_t site, int dir, 
 
 // MODE 0: S2 on every cell of simulation b (READY parents are remembered);  MODE 1: S3 detect by rescanning the map.
 // CTA `rank` of `cs` takes the 16-word tiles rank, rank + cs, ... of the simulation's map and compacts the non-empty map
-// words; then every WARP takes whole words and every LANE one map bit = 8 consecutive sites: one 8-byte load of their
-// states, one 16-byte load of their clocks, six 16-byte loads of their fields, all issued before the first site is
-// worked on, and at most three vector stores back.  Nothing is loaded for a lane whose bit is clear.
+// words; the set bits of 128 such words at a time are expanded into a list of occupied GROUPS (one map bit = 8 consecutive
+// sites), and every THREAD takes one group: one 8-byte load of its states, one 16-byte load of its clocks, six 16-byte loads
+// of its fields, all issued before the first site is worked on, and at most three vector stores back.  (Round 1 gave a
+// warp one map word and a lane one bit: on a 3.5k-cell tumour 9 of 32 lanes had a set bit and 4.5 of 32 lanes were active
+// per instruction of S2 -- ncu, profiles/r02_ncu_cells_divide_c5.txt is the capture before this change.)
 template <int MODE>
 __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int cur, int b, int rank, int cs, uint32_t step,
                                         const uint32_t *__restrict__ occ_b, uint32_t nblk, CDShared &sh, int *__restrict__ err,
@@ -457,10 +462,29 @@ __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int 
         }
         __syncthreads();
         const uint32_t nW = sh.nW;
-        for (uint32_t wi = warp; wi < nW; wi += CD_THREADS / 32) {
-            const uint32_t w = sh.W[wi];
-            if (!((occ_b[w] >> lane) & 1u)) continue;                         // no cell in my 8 sites
-            const uint32_t site0 = w * 256u + 8u * (uint32_t)lane;
+        for (uint32_t c0 = 0; c0 < nW; c0 += CD_GWORDS) {
+            if (tid == 0) sh.nG = 0;
+            __syncthreads();
+            {   // two threads per map word expand its set bits (16 each) into the group list; the order is irrelevant to the result
+                const uint32_t wi = c0 + ((uint32_t)tid >> 1);
+                if (wi < nW) {
+                    const uint32_t w = sh.W[wi];
+                    uint32_t bits = (occ_b[w] >> (16u * ((uint32_t)tid & 1u))) & 0xFFFFu;
+                    if (bits) {
+                        uint32_t pos = atomicAdd(&sh.nG, (uint32_t)__popc(bits));
+                        while (bits) {
+                            const uint32_t bit = (uint32_t)__ffs(bits) - 1u;
+                            bits &= bits - 1u;
+                            sh.G[pos++] = (w << 5) | (bit + 16u * ((uint32_t)tid & 1u));
+                        }
+                    }
+                }
+            }
+            __syncthreads();
+            const uint32_t nG = sh.nG;
+        for (uint32_t gi = tid; gi < nG; gi += CD_THREADS) {
+            const uint32_t ge = sh.G[gi];
+            const uint32_t site0 = (ge >> 5) * 256u + 8u * (ge & 31u);
             const unsigned long long sv = __ldcg(reinterpret_cast<const unsigned long long *>(sb + site0));
             if (MODE == 0) {
                 // Branch-light form of [D S2].  Per step almost every cell only refreshes its mode bits and counts its clock down;
@@ -531,6 +555,8 @@ __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int 
                     if (dir >= 0) cd_winner(sh, site, dir, err, sp, b);
                 }
             }
+        }
+            __syncthreads();                                                  // the group list is rebuilt by the next chunk
         }
         __syncthreads();
     }
