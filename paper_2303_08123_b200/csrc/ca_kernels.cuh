@@ -503,6 +503,7 @@ __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int 
                 uint32_t cn[4] = { cv.x, cv.y, cv.z, cv.w }, dn[4] = { dv.x, dv.y, dv.z, dv.w };
                 unsigned long long sn = sv;
                 bool dm_dirty = false;
+                uint32_t pmask = 0;                                          // bit k: site k is a READY parent after S2; bit 8 + k: known to be blocked
 #pragma unroll
                 for (int k = 0; k < 8; ++k) {
                     const uint32_t s0 = (uint32_t)(sv >> (8 * k)) & 0xFFu, kind = s0 & 7u;
@@ -532,9 +533,15 @@ __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int 
                     }
                     sn = (sn & ~(0xFFull << (8 * k))) | ((unsigned long long)s1 << (8 * k));
                     cn[k >> 1] = (cn[k >> 1] & ~(0xFFFFu << (16 * (k & 1)))) | ((c1 & 0xFFFFu) << (16 * (k & 1)));
-                    if (is_parent(s1)) {
-                        const uint32_t slot = atomicAdd(&sh.nP, 1u);
-                        if (slot < CD_PCAP) sh.Pl[slot] = i | ((s1 & CA_BLOCKED) << 24);
+                    if (is_parent(s1)) pmask |= (1u << k) | ((s1 & CA_BLOCKED) << (8 + k - 7));
+                }
+                // one shared-memory atomic per group, not per parent: the core of a grown tumour is full of blocked READY parents, and
+                // a counter that has passed CD_PCAP (S3 then rescans the map) is left alone
+                if ((pmask & 0xFFu) && *(volatile uint32_t *)&sh.nP <= (uint32_t)CD_PCAP) {
+                    uint32_t slot = atomicAdd(&sh.nP, (uint32_t)__popc(pmask & 0xFFu));
+                    for (uint32_t m = pmask & 0xFFu; m; m &= m - 1u, ++slot) {
+                        const uint32_t k = (uint32_t)__ffs(m) - 1u;
+                        if (slot < CD_PCAP) sh.Pl[slot] = (site0 + k) | (((pmask >> (8 + k)) & 1u) << 31);
                     }
                 }
                 if (sn != sv) *reinterpret_cast<unsigned long long *>(stb + site0) = sn;
