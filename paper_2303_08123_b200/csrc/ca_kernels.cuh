@@ -439,7 +439,7 @@ __device__ __forceinline__ void cd_winner(CDShared &sh, uint32_t site, int dir, 
 // sites), and every THREAD takes one group: one 8-byte load of its states, one 16-byte load of its clocks, six 16-byte loads
 // of its fields, all issued before the first site is worked on, and at most three vector stores back.  (Round 1 gave a
 // warp one map word and a lane one bit: on a 3.5k-cell tumour 9 of 32 lanes had a set bit and 4.5 of 32 lanes were active
-// per instruction of S2 -- ncu, profiles/r02_ncu_cells_divide_c5.txt is the capture before this change.)
+// per instruction of S2 -- ncu, profiles/r02_ncu_cells_divide_c5_before_regrouping.txt is the capture before this change.)
 template <int MODE>
 __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int cur, int b, int rank, int cs, uint32_t step,
                                         const uint32_t *__restrict__ occ_b, uint32_t nblk, CDShared &sh, int *__restrict__ err,
