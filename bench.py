@@ -58,15 +58,16 @@ def ncu_traffic(pattern):
     import re
     files = sorted(glob.glob(os.path.join(ROOT, "profiles", pattern)))
     if not files:
-        return None, None
+        return None, None, None
     txt = open(files[-1]).read()
     tot = 0.0
     for key in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
         m = re.search(key + r"\s+([0-9.]+)\s+(\w+)", txt)
         if not m:
-            return None, None
+            return None, None, None
         tot += float(m.group(1)) * {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}.get(m.group(2), 0.0)
-    return tot, "profiles/" + os.path.basename(files[-1])
+    m = re.search(r"--batch (\d+)", txt)
+    return tot, "profiles/" + os.path.basename(files[-1]), (int(m.group(1)) if m else None)
 
 
 class ClockSampler:
@@ -250,11 +251,13 @@ def roofline_block(kernel, B, sites, stage_ms, per_stage_launches, step_ms_per_c
     launch_ms = stage_ms / per_stage_launches
     alg = B_ALG * B * sites / per_stage_launches          # 25 B x sites x (CA steps one launch completes)
     achieved = alg / (launch_ms * 1e-3) / 1e9
-    traffic, src = ncu_traffic(traffic_pattern) if traffic_pattern else (None, None)
+    traffic, src, tb = ncu_traffic(traffic_pattern) if traffic_pattern else (None, None, None)
     return {"bound": "hbm", "kernel": kernel + ": diffusion-reaction stage S1, all n_sub sub-steps (%d launch(es) per CA step)" % round(per_stage_launches),
             "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
             "launch_ms": launch_ms, "algorithmic_bytes_per_launch": alg,
-            "traffic": traffic, "traffic_source": (src + " (an earlier ncu --set full capture, at the batch that file names; not measured in this run)") if src else None,
+            "traffic": traffic, "traffic_batch": tb,
+            "traffic_over_algorithmic": (traffic / (B_ALG * tb * sites)) if (traffic and tb) else None,
+            "traffic_source": (src + " (an earlier ncu --set full capture, at the batch that file names; not measured in this run)") if src else None,
             "stage_share_of_step": stage_ms / step_ms_per_ca_step if step_ms_per_ca_step else None,
             "whole_step_frac": (B_ALG * B * sites / (step_ms_per_ca_step * 1e-3) / 1e9) / peak if step_ms_per_ca_step else None}
 
@@ -523,7 +526,7 @@ def run_ours(args):
 
     # ---- dominant kernel alone
     stage_ms, nl = time_stage(torch, g, stream, 10 if B >= 4096 else 30)
-    roofline = roofline_block("k_diffuse_fused", B, sites, stage_ms, nl, ms_per_step / S, "r*_ncu_fused_*.txt")
+    roofline = roofline_block("k_diffuse_fused", B, sites, stage_ms, nl, ms_per_step / S, "r02_ncu_fused_*.txt")
 
     # ---- end to end through the C ABI with HOST buffers over the SAME simulated window: every step uploads the protocol
     #      table as it stands (pinned host memory -> device) and reads the fitness back to the host

@@ -145,3 +145,27 @@ def test_the_callers_current_device_is_left_alone():
     g.step(2)
     assert torch.cuda.current_device() == 0
     g.close()
+
+
+def test_get_option_reports_the_diffusion_kernel_that_serves_a_lattice():
+    """ca_get_option: 1 k_diffuse_fused (planes <= 64^2), 3 k_diffuse_rows (96- / 80-wide), 2 k_diffuse_slab (other widths that are
+    multiples of 16), 0 the per-sub-step fallback; knobs read back what was set."""
+    p = w.default_params()
+    for dims, kern in (((64, 64, 8), 1), ((32, 32, 8), 1), ((96, 96, 8), 3), ((80, 80, 8), 3), ((96, 40, 8), 3), ((128, 72, 8), 2), ((37, 21, 8), 0), ((100, 100, 8), 0)):
+        g = binding.CaBatch(1, *dims, p)
+        assert g.get_option("diffusion_kernel") == kern, (dims, g.get_option("diffusion_kernel"))
+        g.set_option("fused", 0)
+        assert g.get_option("diffusion_kernel") == 0
+        g.close()
+    g = binding.CaBatch(2, 96, 96, 8, p)
+    assert g.get_option("rows_cluster") == 0 and g.get_option("graph_steps") == 20
+    g.set_option("rows_cluster", 3)
+    g.set_option("graph_steps", 4)
+    assert g.get_option("rows_cluster") == 3 and g.get_option("graph_steps") == 4
+    with pytest.raises(binding.CaError):
+        g.get_option("no_such_option")
+    g.close()
+    g = binding.CaBatch(1, 80, 80, 8, p)
+    with pytest.raises(binding.CaError):
+        g.set_option("rows_cluster", 3)              # clusters of 3 exist for 96 x 96 planes only
+    g.close()
