@@ -317,10 +317,10 @@ struct Fused {
     template <int PH, bool STEADY>
     static __device__ __forceinline__ void step(const int i, u64 (&h)[NL][3][F_PY], FusedCtx &c)
     {
-        // most strips of most planes hold no cell: a copy of the steady iteration without any source-term code keeps the
-        // hot loop short (instruction cache) and branch-free
-        if (STEADY && ((c.flags & ((1u << NL) - 1u)) | c.slowmask) == 0u) step_body<PH, true, true>(i, h, c);
-        else step_body<PH, STEADY, false>(i, h, c);
+        // Round 1 kept a second copy of the steady iteration without any source-term code for strips that hold no cell.  One
+        // body per phase is faster (round 2: configs[1] step 130.3 -> 127.9 us on 3k-cell tumours, 210.5 -> 205.0 us on 1.1e5-cell
+        // ones): the untaken, warp-uniform branches cost less than the instruction-cache misses of six hot bodies.
+        step_body<PH, STEADY, false>(i, h, c);
     }
 
     template <int PH, bool STEADY, bool NOCELLS>

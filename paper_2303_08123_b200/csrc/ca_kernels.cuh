@@ -445,7 +445,7 @@ __device__ __forceinline__ void cd_pass(const KParams &P, const Lattice &L, int 
                                         const uint32_t *__restrict__ occ_b, uint32_t nblk, CDShared &sh, int *__restrict__ err,
                                         int *__restrict__ lys_b, bool trust, const SpillArgs &sp)
 {
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tid = threadIdx.x;
     const long long sbase = (long long)b * P.n;
     const uint8_t *sb = L.state + sbase;
     uint8_t *stb = L.state + sbase;
