@@ -40,6 +40,15 @@ def welch_t(a, b):
     return float(t), float(df), p
 
 
+def _kolmogorov_sf(lam):
+    """Q_KS(lambda) = 2 * sum_{k>=1} (-1)^(k-1) exp(-2 k^2 lambda^2); the alternating series does not converge for small
+    lambda (it is 1 there to every digit), so identical samples (D = 0) get p = 1, not the series' 0."""
+    if lam < 0.3:
+        return 1.0
+    p = 2.0 * sum((-1) ** (k - 1) * math.exp(-2.0 * (k * lam) ** 2) for k in range(1, 101))
+    return float(min(1.0, max(0.0, p)))
+
+
 def ks_2samp(a, b):
     """Two-sample Kolmogorov-Smirnov statistic D and its asymptotic p-value."""
     a, b = np.sort(np.asarray(a, np.float64)), np.sort(np.asarray(b, np.float64))
@@ -49,8 +58,7 @@ def ks_2samp(a, b):
     d = float(np.abs(cdfa - cdfb).max())
     en = math.sqrt(len(a) * len(b) / (len(a) + len(b)))
     lam = (en + 0.12 + 0.11 / en) * d
-    p = 2.0 * sum((-1) ** (k - 1) * math.exp(-2.0 * (k * lam) ** 2) for k in range(1, 101))
-    return d, float(min(1.0, max(0.0, p)))
+    return d, _kolmogorov_sf(lam)
 
 
 def same_distribution(a, b, alpha=0.01):
@@ -86,8 +94,7 @@ def ks_normality(a, discrete=False):
         d = float(max((np.arange(1, n + 1) / n - cdf).max(), (cdf - np.arange(0, n) / n).max()))
     en = math.sqrt(n)
     lam = (en + 0.12 + 0.11 / en) * d
-    p = 2.0 * sum((-1) ** (k - 1) * math.exp(-2.0 * (k * lam) ** 2) for k in range(1, 101))
-    return d, float(min(1.0, max(0.0, p)))
+    return d, _kolmogorov_sf(lam)
 
 
 def mean_ci95(a):

@@ -68,3 +68,17 @@ def test_compare_implementations_and_pvalue_pile_up():
     assert not stats.pvalues_not_piled_up(stats.compare_implementations(x, z)["p_t"])
     m, ci = stats.mean_ci95(np.arange(10.0))
     assert m == 4.5 and abs(ci - st.t.ppf(0.975, 9) * np.arange(10.0).std(ddof=1) / np.sqrt(10)) < 1e-12
+
+
+def test_identical_samples_are_the_same_distribution():
+    """D = 0 must give p = 1 (the alternating Kolmogorov series is 0 there if summed naively): a GPU run that reproduces
+    the oracle's counts exactly is the best possible agreement, not a rejection."""
+    x = np.array([1828.0, 1683.0, 1808.0, 1733.0, 1658.0])
+    assert stats.ks_2samp(x, x.copy()) == (0.0, 1.0)
+    assert stats.welch_t(x, x.copy())[2] == 1.0
+    assert stats.same_distribution(x, x.copy())
+    rng = np.random.default_rng(3)
+    a, b = rng.normal(0, 1, 400), rng.normal(0.02, 1, 400)
+    ref = st.ks_2samp(a, b)
+    d, p = stats.ks_2samp(a, b)
+    assert abs(d - ref.statistic) < 1e-12 and abs(p - ref.pvalue) < 0.05
