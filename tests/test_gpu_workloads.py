@@ -187,8 +187,9 @@ def test_long_horizon_statistical_parity_with_the_fp64_oracle_ensemble():
             assert stats.same_distribution(x[k], y[k]), (name, k, cmp["p_t"][k], cmp["p_ks"][k])
         assert stats.pvalues_not_piled_up(cmp["p_t"]), (name, cmp["p_t"])
     # the trajectories share their random streams: most simulations still agree exactly with the fp64 oracle after 75 600 steps
+    # (measured in round 2: all 240 agree exactly, live and occupied; a threshold flip would show up here first)
     same = float((gpu_occ == ref_occ).mean())
-    assert same > 0.5, same
+    assert same > 0.9, same
 
 
 def test_next3_paper_geometry_library_fitness_methodology_and_whole_run_parity():
