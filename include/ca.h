@@ -68,6 +68,9 @@ typedef struct ca_params {
     int32_t repair_period, repair_shift;   /* integer repair law [D G11] */
     int32_t lysis_steps;         /* steps a DEAD cell keeps its site [D G12] */
     int32_t N_ref;               /* Eq. 1 constant (paper: 1500); 0 => number of interior sites [D G14] */
+    int32_t well_mixed_medium;   /* != 0: every EMPTY site is held at the medium values ("well-mixed replenished substrate",
+                                    PAPER.md l.244; the alternative reading of [D G2], for the paper-shaped workload NEXT-3).
+                                    Served by the per-sub-step diffusion kernel (the fused kernels assume free diffusion). */
 } ca_params;
 
 /* Initial spheroid [D S-SEED]: kind 0 SINGLE cell, 1 CLUSTER7 (centre + 6 face neighbours,

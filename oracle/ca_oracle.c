@@ -266,6 +266,8 @@ static void diffuse_once(car_ctx *c)
                 for (int x = 0; x < nx; ++x) {
                     int64_t i = ((int64_t)z * ny + y) * nx + x;
                     if (is_wall(c, x, y, z)) { b[i] = a[i]; continue; }
+                    /* alternative reading of G2 ("well-mixed replenished substrate"): an EMPTY site is medium */
+                    if (c->p.well_mixed_medium && ST_KIND(c->state[i]) == K_EMPTY) { b[i] = (real)c->p.boundary[s]; continue; }
                     real sum6 = ((a[i - sx] + a[i + sx]) + (a[i - sy] + a[i + sy])) + (a[i - sz] + a[i + sz]);
                     real six  = (real)6 * a[i];
                     real lap  = sum6 - six;

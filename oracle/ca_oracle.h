@@ -61,6 +61,7 @@ typedef struct {
     int32_t repair_period, repair_shift;   /* G11 */
     int32_t lysis_steps;         /* G12 */
     int32_t N_ref;               /* Eq. 1 constant; 0 => interior sites (G14) */
+    int32_t well_mixed_medium;   /* != 0: EMPTY sites are held at the medium values (alternative reading of G2) */
 } car_params;
 
 typedef struct { int32_t kind; int32_t cx, cy, cz; float radius; int32_t shared_init; } car_init;

@@ -33,7 +33,7 @@ class CaParams(C.Structure):
         ("alpha", C.c_float * 4), ("beta", C.c_float * 4),
         ("oer_m", C.c_float), ("oer_K", C.c_float),
         ("repair_period", C.c_int32), ("repair_shift", C.c_int32),
-        ("lysis_steps", C.c_int32), ("N_ref", C.c_int32),
+        ("lysis_steps", C.c_int32), ("N_ref", C.c_int32), ("well_mixed_medium", C.c_int32),
     ]
 
 
@@ -105,6 +105,7 @@ def make_params(d):
         p.J[k] = int(d["J"][k])
         p.alpha[k] = d["alpha"][k]
         p.beta[k] = d["beta"][k]
+    p.well_mixed_medium = int(d.get("well_mixed_medium", 0))
     for k in ("repair_period", "repair_shift", "lysis_steps", "N_ref"):
         setattr(p, k, int(d[k]))
     return p

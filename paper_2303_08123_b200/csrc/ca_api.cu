@@ -370,6 +370,7 @@ int ca_create(ca_ctx **out, int batch, int nx, int ny, int nz, const ca_params *
     for (int k = 0; k < 4; ++k) { P.T[k] = p->T[k]; P.J[k] = p->J[k]; P.alpha[k] = p->alpha[k]; P.beta[k] = p->beta[k]; }
     P.oer_m = p->oer_m; P.oer_K = p->oer_K; P.repair_period = p->repair_period; P.repair_shift = p->repair_shift;
     P.lysis_steps = p->lysis_steps; P.N_ref = p->N_ref; P.key0 = P.key1 = 0; P.sim_id_base = 0;
+    P.well_mixed = p->well_mixed_medium != 0;
     c->Y = make_layout(batch, n, max_frac);
     c->ws = (uint8_t *)workspace;
     for (int bsel = 0; bsel < 2; ++bsel) for (int s = 0; s < 3; ++s) c->L.f[bsel][s] = (float *)(c->ws + c->Y.field[bsel][s]);

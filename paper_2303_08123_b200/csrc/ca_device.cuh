@@ -28,6 +28,7 @@ struct KParams {
     int repair_period, repair_shift;
     int lysis_steps;
     int N_ref;
+    int well_mixed;              // != 0: EMPTY sites are held at the medium values [D G2, alternative reading]
     uint32_t key0, key1;         // Philox key = rng_seed (low, high)
     uint32_t sim_id_base;
 };

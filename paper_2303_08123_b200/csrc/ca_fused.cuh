@@ -784,6 +784,7 @@ inline void fused_configure(const KParams &P, FusedPlan &F)
     F.ok = false;
     F.tiled = (P.nx > 64 || P.ny > 64);
     if (P.nz < 3 || P.n_sub < 1 || P.n_sub > 2 * F_MAXNL || P.nx < 4) return;
+    if (P.well_mixed) return;                                     // EMPTY sites pinned at the medium values: the per-sub-step kernel serves that reading
     FusedGeom G{};
     F.rows = F.tiled && rows_configure(P, F);
     if (F.rows) {

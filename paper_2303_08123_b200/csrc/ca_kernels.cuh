@@ -108,6 +108,11 @@ __global__ void k_diffuse_sub(KParams P, Lattice L, int src)
         return;
     }
     const uint32_t st = L.state[gi];
+    if (P.well_mixed && (st & 7u) == CA_EMPTY) {                              // well-mixed medium: an EMPTY site is held at the medium values
+#pragma unroll
+        for (int s = 0; s < 3; ++s) L.f[dst][s][gi] = P.boundary[s];
+        return;
+    }
     const bool lv = is_live(st);
     const int mode = (st >> 3) & 3;
     const long long sy = P.nx, sz = (long long)P.nx * P.ny;

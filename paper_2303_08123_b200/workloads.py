@@ -43,6 +43,7 @@ _DEFAULT = {
     "repair_period": 60, "repair_shift": 4,
     "lysis_steps": 14400,
     "N_ref": 0,
+    "well_mixed_medium": 0,                        # 1: EMPTY sites held at the medium values (alternative reading of G2; NEXT-3)
 }
 
 
@@ -160,8 +161,9 @@ def paper_geometry():
     interior plane of 38 x 38 = 1 444 sites between two planes of medium, so that every site touches the replenished
     medium (l.244) -- N_ref = 1500, a 9-site seed (BALL r = 1.5 in the plane), 10 tumours that differ by their simulation
     id, 240 h of growth, 240 h of evaluation, BMI and BMII of the paper (l.49) plus an untreated control, 8 seeds per
-    tumour (80 samples per protocol, l.282).  Not reproduced: ~20 cells per site (this build keeps one cell per site,
-    DESIGN.md G1) and the paper's calibrated parameters (it prints none)."""
+    tumour (80 samples per protocol, l.282); run with `well_mixed_medium = 1` (EMPTY sites are medium, l.244).  Not
+    reproduced: ~20 cells per site (this build keeps one cell per site, G1) and the paper's calibrated
+    parameters (it prints none)."""
     seed = MASTER_SEED + 30
     names = ["untreated", "BMI", "BMII"]
     F = 8

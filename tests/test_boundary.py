@@ -52,7 +52,7 @@ def test_create_rejects_bad_arguments_without_a_gpu(lib):
 
 
 def test_struct_layouts():
-    assert C.sizeof(binding.CaParams) == 4 * (2 + 3 + 3 + 12 + 5 + 4 + 4 + 4 + 4 + 2 + 2 + 1 + 1)
+    assert C.sizeof(binding.CaParams) == 4 * (2 + 3 + 3 + 12 + 5 + 4 + 4 + 4 + 4 + 2 + 2 + 1 + 1 + 1)      # ... + well_mixed_medium
     assert C.sizeof(binding.CaInit) == 24
 
 

@@ -199,7 +199,7 @@ def test_next3_paper_geometry_library_fitness_methodology_and_whole_run_parity()
     simulations is re-run WHOLE (144 000 steps) by the fp32 build of the oracle from the same library snapshot: same counts."""
     from paper_2303_08123_b200 import ga
     cfg = w.paper_geometry()
-    p = w.default_params(N_ref=cfg["n_ref"])
+    p = w.default_params(N_ref=cfg["n_ref"], well_mixed_medium=1)     # "well-mixed replenished substrate" (l.244): EMPTY sites are medium
     dims = cfg["dims"]
     lib = pregrow.grow_library(dims, p, cfg["init"], cfg["rng_seed"], cfg["n_tumours"], cfg["grow_h"])
     occ0 = np.array([int((((s["state"] & 7) >= 1) & ((s["state"] & 7) <= 5)).sum()) for s in lib])
@@ -223,4 +223,35 @@ def test_next3_paper_geometry_library_fitness_methodology_and_whole_run_parity()
     r.run(cfg["grow_h"] + cfg["horizon_h"])
     assert cnt[b].tolist() == r.counts().tolist()
     assert fit[pr, j, s] == r.fitness()
+    g.close()
+
+
+@pytest.mark.parametrize("dims", [(20, 14, 9), (40, 40, 3)])
+def test_well_mixed_medium_flag_matches_the_oracle(dims):
+    """The alternative reading of G2 (EMPTY sites held at the medium values) on the GPU: a 60-step stress window with
+    irradiation, divisions, deaths and lysis, bit for bit against the fp32 build of the oracle and <= 1e-4 against fp64."""
+    p = w.stress_params(well_mixed_medium=1)
+    seed = 0x5EED77
+    g = binding.CaBatch(3, *dims, p, max_frac=2)
+    assert g.get_option("diffusion_kernel") == 0                   # served by the per-sub-step kernel
+    c = (dims[0] // 2, dims[1] // 2, dims[2] // 2)
+    g.seed("ball", center=c, radius=3.0, rng_seed=seed, sim_id_base=4)
+    dose = np.array([[3.0, 2.0], [6.0, 1.5], [0.5, 4.0]])
+    delay = np.array([[0.01, 0.03], [0.0, 0.05], [0.02, 0.02]])
+    g.set_protocols(dose, delay)
+    g.step(60)
+    for b in range(3):
+        gs = g.get_state(b)
+        for prec in ("f32", "f64"):
+            r = o.OracleSim(*dims, p, precision=prec)
+            r.seed("ball", center=c, radius=3.0, rng_seed=seed, sim_id=4 + b)
+            r.set_protocol(dose[b], delay[b])
+            r.step(60)
+            assert_ints_equal(gs, r.get_state(), "%s sim %d" % (prec, b))
+            if prec == "f32":
+                assert_fields_bitwise(gs, r.get_state(), "f32 sim %d" % b)
+            else:
+                assert_fields_close(gs, r.get_state(), p, 1e-4, "f64 sim %d" % b)
+    st = g.get_state(0)
+    assert np.all(st["glc"][(st["state"] & 7) == 0] == np.float32(p["boundary"][1]))      # EMPTY sites: exactly the medium value
     g.close()

@@ -187,3 +187,41 @@ def test_p6_mass_balance_and_maximum_principle():
             else:
                 assert b[name].min() >= cb
             assert b[name].min() > 0.0          # no clamp fired
+
+
+def test_well_mixed_medium_closed_forms_and_pinned_empty_sites():
+    """Alternative reading of G2 ("well-mixed replenished substrate"; the `well_mixed_medium` flag of
+    NEXT-3): every EMPTY site is held at the medium value.  Closed forms that do not re-use the oracle's formula:
+    an isolated consuming cell sees six medium neighbours, so its fixed point is c* = c_b + r / (6 lambda);
+    two face-adjacent identical cells see five medium neighbours and each other: c* = c_b + r / (5 lambda).
+    EMPTY sites stay at the boundary value bit for bit; without the flag they do not."""
+    n = 9
+    p = w.default_params(well_mixed_medium=1)
+    b = np.asarray(p["boundary"], np.float32).astype(np.float64)
+    lam = np.asarray(p["lambda"], np.float32).astype(np.float64)
+    rate = np.asarray(p["rate"], np.float32).astype(np.float64)
+    shape = (n, n, n)
+    for cells, nb in (([(4, 4, 4)], 6.0), ([(4, 4, 4), (4, 4, 5)], 5.0)):
+        st = blank_state(n, n, n)
+        for c in cells:
+            st[c] = K_G1                                      # mode bits 0 = PA
+        f = const_fields(p, shape)
+        sim = o.OracleSim(n, n, n, p)
+        sim.set_state(state=st, clock=np.full(shape, 1000, np.uint16), damage=np.zeros(shape, np.uint16), o2=f[0], glc=f[1], h=f[2], step=0)
+        sim.diffuse_substeps(400)
+        out = sim.get_state()
+        for s, name in enumerate(("o2", "glc", "h")):
+            expect = b[s] + rate[s][0] / (nb * lam[s])
+            for c in cells:
+                assert abs(out[name][c] - expect) <= 1e-12 * abs(expect), (name, c, out[name][c], expect)
+            empty = (st == 0)
+            assert np.array_equal(out[name][empty], np.full(empty.sum(), b[s]))       # pinned, bitwise
+    # the same isolated cell WITHOUT the flag: its neighbours are depleted (free diffusion), the centre lies lower
+    p0 = w.default_params()
+    st = blank_state(n, n, n); st[4, 4, 4] = K_G1
+    f = const_fields(p0, shape)
+    sim = o.OracleSim(n, n, n, p0)
+    sim.set_state(state=st, clock=np.full(shape, 1000, np.uint16), damage=np.zeros(shape, np.uint16), o2=f[0], glc=f[1], h=f[2], step=0)
+    sim.diffuse_substeps(400)
+    out = sim.get_state()
+    assert out["glc"][4, 4, 5] < b[1] and out["glc"][4, 4, 4] < b[1] + rate[1][0] / (6.0 * lam[1])
