@@ -315,7 +315,7 @@ def config_probe(torch, binding, name, cfg, params, snap, device, ca_steps, kern
     return out
 
 
-def full_horizon(torch, binding, cfg, params, snap, device):
+def full_horizon(torch, binding, cfg, params, snap, device, label="configs[1]"):
     """evaluate the whole workload to its horizon once: MEASURED protocols/hour, upload and readout included"""
     B = cfg["batch"]
     nx, ny, nz = cfg["dims"]
@@ -331,7 +331,7 @@ def full_horizon(torch, binding, cfg, params, snap, device):
     fit = g.fitness()
     dt = time.perf_counter() - t0
     cnt = g.counts()
-    out = {"workload": "BASELINE configs[1] whole job: %d protocols x %dx%dx%d to %g h" % (B, nx, ny, nz, cfg["horizon_h"]),
+    out = {"workload": "BASELINE %s whole job: %d protocols x %dx%dx%d to %g h" % (label, B, nx, ny, nz, cfg["horizon_h"]),
            "protocols_per_hour": B * 3600.0 / dt, "seconds": dt, "ca_steps": steps, "us_per_ca_step": dt / steps * 1e6,
            "site_updates_per_s": B * nx * ny * nz * steps / dt, "whole_job_frac_of_hbm_roofline": B_ALG * B * nx * ny * nz * steps / dt / 1e9 / measured_peaks()[0],
            "fitness_min_mean_max": [float(fit.min()), float(fit.mean()), float(fit.max())],
@@ -442,6 +442,25 @@ def run_probe(args):
     opts = {} if args.rows_cluster is None else {"rows_cluster": args.rows_cluster}
     out = config_probe(torch, binding, str(k - 1), cfg, params, snap, 0, args.ca_steps or (200 if k == 2 else 20), kern, None, options=opts)
     out["probe"] = {"config": args.probe, "batch": cfg["batch"], "tumour_radius": args.tumour_radius}
+    print(json.dumps(out))
+
+
+def run_whole_job(args):
+    """--whole-job c2|c3|c4: evaluate that configuration's WHOLE job once (all its protocols to the horizon) and print the
+    measured protocols/hour.  configs[2] / [3] take about an hour of GPU time each; not part of the default run."""
+    import torch
+    from paper_2303_08123_b200 import binding, pregrow
+    torch.cuda.set_device(0)
+    params = w.default_params()
+    k = {"c2": 2, "c3": 3, "c4": 4}[args.whole_job]
+    cfg = dict(w.config(k))
+    if k == 3:
+        snap, grown_h = pregrow.grow(cfg["dims"], params, cfg["init"], cfg["rng_seed"], target_extent=cfg["pregrow_diameter"], check_h=24.0)
+        cfg["t0_h"] = grown_h
+    else:
+        snap = warm_snapshot(binding, cfg, params, 0)
+    out = full_horizon(torch, binding, cfg, params, snap, 0, label="configs[%d]" % (k - 1))
+    out["metric"] = "protocols_per_hour_measured"
     print(json.dumps(out))
 
 
@@ -628,6 +647,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--probe", default=None, choices=["c2", "c3", "c4"], help="measure ONE configuration alone (with --batch: reduced batch) and print its per_config entry")
     ap.add_argument("--tumour-radius", type=float, default=None, help="--probe only: start from a seeded BALL of this radius (late, dense phase)")
+    ap.add_argument("--whole-job", default=None, choices=["c2", "c3", "c4"], help="run that configuration's whole job once and print the measured protocols/hour (c3, c4: about an hour each)")
     ap.add_argument("--rows-cluster", type=int, default=None, help="--probe c3 only: 0 = slabs with a halo, 3 = clusters of 3 CTAs per plane")
     ap.add_argument("--ga", action="store_true", help="configs[4] sharded population evaluation + host GA loop at reduced size")
     ap.add_argument("--ga-population", type=int, default=128)
@@ -637,7 +657,9 @@ def main():
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
-    if args.probe:
+    if args.whole_job:
+        run_whole_job(args)
+    elif args.probe:
         run_probe(args)
     elif args.ga:
         run_ga(args)
