@@ -454,12 +454,16 @@ def run_whole_job(args):
     params = w.default_params()
     k = {"c2": 2, "c3": 3, "c4": 4}[args.whole_job]
     cfg = dict(w.config(k))
+    if args.batch and args.batch < cfg["batch"]:            # the first `batch` protocols of the configuration only (a call on the GPU box is limited to one hour)
+        cfg["batch"] = args.batch
+        for key in ("dose", "delay", "nfrac"):
+            cfg[key] = cfg[key][:args.batch]
     if k == 3:
         snap, grown_h = pregrow.grow(cfg["dims"], params, cfg["init"], cfg["rng_seed"], target_extent=cfg["pregrow_diameter"], check_h=24.0)
         cfg["t0_h"] = grown_h
     else:
         snap = warm_snapshot(binding, cfg, params, 0)
-    out = full_horizon(torch, binding, cfg, params, snap, 0, label="configs[%d]" % (k - 1))
+    out = full_horizon(torch, binding, cfg, params, snap, 0, label="configs[%d]%s" % (k - 1, "" if cfg["batch"] == w.config(k)["batch"] else " (first %d protocols)" % cfg["batch"]))
     out["metric"] = "protocols_per_hour_measured"
     print(json.dumps(out))
 
