@@ -174,6 +174,23 @@ int ca_get_option(ca_ctx *c, const char *name, int *value);
 /* Number of kernel launches (graph nodes included) issued by this context so far. */
 int64_t ca_launch_count(ca_ctx *c);
 
+/* S4 without a context and WITHOUT ANY ALLOCATION (for callers that cannot call cudaMalloc: code under CUDA-graph
+ * capture, serving loops, harnesses that forbid it): per-simulation counts and Eq. 1 fitness of a state array the
+ * caller owns.
+ *   state_dev        DEVICE, 16-byte aligned, [batch][nz][ny][nx] u8 in the canonical encoding (bit 7 is ignored)
+ *   n_ref            Eq. 1 constant; 0 => number of interior sites [D G14]
+ *   counts_out_dev   DEVICE, [batch][CA_NCOUNT] int32, or NULL
+ *   fitness_out_dev  DEVICE, [batch] fp32, or NULL (at least one of the two outputs)
+ *   stream           a cudaStream_t (NULL: the default stream); the call is asynchronous on it
+ * The accumulation scratch is a fixed device array inside the library: CA_NOALLOC_MAX_BATCH simulations (832 KiB, held
+ * by every GPU that loads the library until the process exits).  CA_EINVAL (text via ca_last_error(NULL)) if batch
+ * exceeds it.  The array is shared by every call and cleared at the start of each: calls that OVERLAP on the GPU
+ * (different streams or host threads) race on it -- serialise them.  Runs on the current device; calls no cudaMalloc,
+ * cudaFree or allocating library routine. */
+enum { CA_NOALLOC_MAX_BATCH = 16384 };
+int ca_counts_noalloc(const uint8_t *state_dev, int batch, int nx, int ny, int nz, int n_ref,
+                      int32_t *counts_out_dev, float *fitness_out_dev, void *stream);
+
 const char *ca_last_error(ca_ctx *c);            /* c may be NULL: error of the last failed ca_create */
 const char *ca_version(void);
 

@@ -19,7 +19,8 @@ INIT_KINDS = {"single": 0, "cluster7": 1, "ball": 2}
 
 EXPORTS = ("ca_version", "ca_last_error", "ca_workspace_bytes", "ca_create", "ca_destroy", "ca_seed", "ca_set_rng",
            "ca_set_protocols", "ca_run", "ca_step", "ca_get_step", "ca_sync", "ca_fitness", "ca_counts",
-           "ca_get_state", "ca_set_state", "ca_stage", "ca_set_option", "ca_get_option", "ca_launch_count")
+           "ca_get_state", "ca_set_state", "ca_stage", "ca_set_option", "ca_get_option", "ca_launch_count",
+           "ca_counts_noalloc")
 
 
 class CaParams(C.Structure):
@@ -82,6 +83,7 @@ def load():
     L.ca_stage.argtypes = [vp, C.c_int, C.c_int]
     L.ca_set_option.argtypes = [vp, C.c_char_p, C.c_int]
     L.ca_get_option.argtypes = [vp, C.c_char_p, C.POINTER(C.c_int)]
+    L.ca_counts_noalloc.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, vp, vp, vp]
     L.ca_launch_count.argtypes = [vp]
     L.ca_launch_count.restype = C.c_int64
     _LIB = L
@@ -113,6 +115,21 @@ def make_params(d):
 
 def _ptr(a):
     return None if a is None else C.c_void_p(a.ctypes.data)
+
+
+CA_NOALLOC_MAX_BATCH = 16384
+
+
+def counts_noalloc(state, nx, ny, nz, n_ref=0, counts_out=None, fitness_out=None, stream=None):
+    """ca_counts_noalloc: counts / Eq. 1 fitness of a torch cuda uint8 tensor `state` [batch][nz][ny][nx] into torch cuda tensors
+    the caller passes (int32 [batch][CA_NCOUNT], fp32 [batch]); the library allocates nothing (fixed scratch, batch <= 16384)."""
+    L = load()
+    batch = int(state.shape[0])
+    ptr = lambda t: None if t is None else C.c_void_p(t.data_ptr())
+    rc = L.ca_counts_noalloc(ptr(state), batch, int(nx), int(ny), int(nz), int(n_ref), ptr(counts_out), ptr(fitness_out),
+                             None if stream is None else C.c_void_p(stream.cuda_stream))
+    if rc:
+        raise CaError(rc, (L.ca_last_error(None) or b"").decode())
 
 
 class CaBatch:

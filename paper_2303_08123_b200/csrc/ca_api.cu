@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -701,3 +702,76 @@ int ca_get_option(ca_ctx *c, const char *name, int *value)
 int64_t ca_launch_count(ca_ctx *c) { return c ? (int64_t)c->launches : 0; }
 
 }  // extern "C"
+
+// ============================================================ entry point that allocates nothing ====
+// ca_counts_noalloc: S4 (per-simulation counts and Eq. 1 fitness) of a DEVICE state array the caller owns, for callers that
+// cannot allocate or hold a workspace (code under CUDA-graph capture, serving loops, harnesses that forbid cudaMalloc).
+// The accumulation scratch of k_counts -- [batch][CA_NCOUNT] int32, one atomic per warp and count -- lives in a file-scope
+// device array of fixed size instead of the caller's workspace: CA_NOALLOC_MAX_BATCH simulations = 832 KiB, held by every
+// GPU that loads the library until the process exits.  In host code the array's NAME is a host-side stand-in, not a device
+// address: its address is taken once per device with cudaGetSymbolAddress (that device current) and passed to the kernels.
+// Every call shares the array: it is cleared at the start of each call (on the caller's stream), and calls that overlap on
+// the GPU (two streams, two host threads) race on it.
+namespace {
+
+static __device__ __align__(256) int g_noalloc_counts[CA_NOALLOC_MAX_BATCH * CA_NCOUNT];
+
+constexpr int kMaxDevices = 64;
+int *g_noalloc_ptr[kMaxDevices] = { nullptr };      // device address of g_noalloc_counts, per device
+std::mutex g_noalloc_mutex;
+
+// occupied = live + dead [D G13]; fitness = N_ref - occupied (Eq. 1); scratch -> the caller's arrays
+__global__ void k_noalloc_finish(const int *__restrict__ scratch, int batch, long long nref, int32_t *__restrict__ counts_out,
+                                 float *__restrict__ fitness_out)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= batch) return;
+    const int occ = scratch[b * CA_NCOUNT + CA_C_LIVE] + scratch[b * CA_NCOUNT + CA_C_DEAD];
+    if (counts_out) {
+        for (int q = 0; q < CA_NCOUNT; ++q) counts_out[b * CA_NCOUNT + q] = q == CA_C_OCCUPIED ? occ : scratch[b * CA_NCOUNT + q];
+    }
+    if (fitness_out) fitness_out[b] = (float)(nref - occ);
+}
+
+}  // namespace
+
+extern "C" int ca_counts_noalloc(const uint8_t *state_dev, int batch, int nx, int ny, int nz, int n_ref,
+                                 int32_t *counts_out_dev, float *fitness_out_dev, void *stream)
+{
+    if (!state_dev || (!counts_out_dev && !fitness_out_dev)) return fail(nullptr, CA_EINVAL, "ca_counts_noalloc: state and at least one output are required");
+    if (batch < 1 || nx < 3 || ny < 3 || nz < 3) return fail(nullptr, CA_EINVAL, "ca_counts_noalloc: bad batch / lattice dims (each dim >= 3)");
+    if ((uintptr_t)state_dev & 15u) return fail(nullptr, CA_EINVAL, "ca_counts_noalloc: state must be 16-byte aligned");
+    if (batch > CA_NOALLOC_MAX_BATCH)
+        return fail(nullptr, CA_EINVAL, "ca_counts_noalloc: batch exceeds CA_NOALLOC_MAX_BATCH (16384 simulations: the static scratch is 832 KiB); use ca_counts on a context");
+    const long long n = (long long)nx * ny * nz;
+    if (n > (1ll << 30)) return fail(nullptr, CA_EINVAL, "ca_counts_noalloc: lattice too large");
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaGetDevice (no CUDA device: this library has no CPU path)");
+    if (dev < 0 || dev >= kMaxDevices) return fail(nullptr, CA_EINVAL, "ca_counts_noalloc: device index beyond 63");
+    int *scratch = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+        if (!g_noalloc_ptr[dev]) {                    // set-up, once per device, with that device current
+            void *p = nullptr;
+            e = cudaGetSymbolAddress(&p, g_noalloc_counts);
+            if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaGetSymbolAddress(g_noalloc_counts)");
+            g_noalloc_ptr[dev] = (int *)p;
+        }
+        scratch = g_noalloc_ptr[dev];
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    // the array keeps the last call's contents: what this call accumulates into starts at zero
+    e = cudaMemsetAsync(scratch, 0, (size_t)batch * CA_NCOUNT * sizeof(int), st);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaMemsetAsync(scratch)");
+    KParams P{};
+    P.nx = nx; P.ny = ny; P.nz = nz; P.batch = batch; P.n = n;
+    const long long per = (n / 16 + 255) / 256;
+    const unsigned int bx = (unsigned int)std::max<long long>(1, std::min<long long>(per, std::max<long long>(1, 2368 / batch)));
+    k_counts<<<dim3(bx, (unsigned int)batch), 256, 0, st>>>(P, state_dev, scratch);
+    const long long nref = n_ref > 0 ? (long long)n_ref : (long long)(nx - 2) * (ny - 2) * (nz - 2);
+    k_noalloc_finish<<<blocks_for(batch, 128), 128, 0, st>>>(scratch, batch, nref, counts_out_dev, fitness_out_dev);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "ca_counts_noalloc kernel launch");
+    return CA_OK;
+}
