@@ -549,7 +549,7 @@ def run_ours(args):
 
     # ---- dominant kernel alone
     stage_ms, nl = time_stage(torch, g, stream, 10 if B >= 4096 else 30)
-    roofline = roofline_block("k_diffuse_fused", B, sites, stage_ms, nl, ms_per_step / S, "r02_ncu_fused_*.txt")
+    roofline = roofline_block("k_diffuse_fused", B, sites, stage_ms, nl, ms_per_step / S, "r02_ncu_fused_c5*.txt")
 
     # ---- end to end through the C ABI with HOST buffers over the SAME simulated window: every step uploads the protocol
     #      table as it stands (pinned host memory -> device) and reads the fitness back to the host
