@@ -440,6 +440,8 @@ def run_probe(args):
         snap = warm_snapshot(binding, cfg, params, 0)
     kern = "k_diffuse_fused" if k == 2 else "k_diffuse_rows"
     opts = {} if args.rows_cluster is None else {"rows_cluster": args.rows_cluster}
+    if args.rows_rp is not None:
+        opts["rows_rp"] = args.rows_rp
     out = config_probe(torch, binding, str(k - 1), cfg, params, snap, 0, args.ca_steps or (200 if k == 2 else 20), kern, None, options=opts)
     out["probe"] = {"config": args.probe, "batch": cfg["batch"], "tumour_radius": args.tumour_radius}
     print(json.dumps(out))
@@ -652,6 +654,7 @@ def main():
     ap.add_argument("--probe", default=None, choices=["c2", "c3", "c4"], help="measure ONE configuration alone (with --batch: reduced batch) and print its per_config entry")
     ap.add_argument("--tumour-radius", type=float, default=None, help="--probe only: start from a seeded BALL of this radius (late, dense phase)")
     ap.add_argument("--whole-job", default=None, choices=["c2", "c3", "c4"], help="run that configuration's whole job once and print the measured protocols/hour (c3, c4: about an hour each)")
+    ap.add_argument("--rows-rp", type=int, default=None, help="--probe c3 only: row pairs per lane of k_diffuse_rows (1 or 2)")
     ap.add_argument("--rows-cluster", type=int, default=None, help="--probe c3 only: 0 = slabs with a halo, 3 = clusters of 3 CTAs per plane")
     ap.add_argument("--ga", action="store_true", help="configs[4] sharded population evaluation + host GA loop at reduced size")
     ap.add_argument("--ga-population", type=int, default=128)

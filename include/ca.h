@@ -163,6 +163,7 @@ int ca_stage(ca_ctx *c, int stage, int arg);
  *   "fused"        1 = temporally fused diffusion kernels (default), 0 = one launch per sub-step
  *   "cell_path"    1 = clustered S2+S3 kernel driven by the occupancy map when the lattice allows (default), 0 = generic scans
  *   "cluster"      CTAs per simulation of the clustered kernel: 1, 2, 4 or 8
+ *   "rows_rp"      k_diffuse_rows on 96-wide planes: 1 = two rows per lane (16 warps), 2 = four rows per lane (8 warps)
  *   "rows_cluster" 3 = k_diffuse_rows as clusters of 3 CTAs per 96 x 96 plane (boundary rows through distributed shared
  *                  memory, no halo), 0 = y-slabs with a halo
  *   "inject_launch_error"  1 = fault injection: the next step / stage call behaves as if a kernel launch had failed

@@ -667,6 +667,10 @@ int ca_set_option(ca_ctx *c, const char *name, int value)
     if (!std::strcmp(name, "inject_launch_error")) {                          // fault injection for the tests: the next step sees a failed kernel launch
         c->launch_err = value ? cudaErrorLaunchOutOfResources : cudaSuccess; return CA_OK;
     }
+    if (!std::strcmp(name, "rows_rp")) {                                       // k_diffuse_rows on 96-wide planes: 1 = two rows per lane, 2 = four
+        if (!((value == 1 || value == 2) && c->fplan.rows && c->P.nx == 96)) return fail(c, CA_EINVAL, "rows_rp must be 1 or 2, on 96-wide planes");
+        c->fplan.rows_rp = value; drop_graphs(c); return CA_OK;
+    }
     if (!std::strcmp(name, "rows_cluster")) {                                  // 0: k_diffuse_rows on slabs with a halo; 3: cluster of 3 CTAs per 96 x 96 plane
         if (!(value == 0 || (value == 3 && c->P.nx == 96 && c->P.ny == 96 && c->fplan.rows))) return fail(c, CA_EINVAL, "rows_cluster must be 0, or 3 on 96 x 96 planes");
         c->fplan.rows_cluster = value; drop_graphs(c); return CA_OK;
@@ -691,6 +695,7 @@ int ca_get_option(ca_ctx *c, const char *name, int *value)
     if (!std::strcmp(name, "cell_path")) { *value = c->cell_path && c->mapped_ok; return CA_OK; }
     if (!std::strcmp(name, "cluster")) { *value = c->cs; return CA_OK; }
     if (!std::strcmp(name, "rows_cluster")) { *value = c->fplan.rows ? c->fplan.rows_cluster : 0; return CA_OK; }
+    if (!std::strcmp(name, "rows_rp")) { *value = c->fplan.rows ? c->fplan.rows_rp : 0; return CA_OK; }
     if (!std::strcmp(name, "rows_nclusters")) { *value = c->fplan.nclusters; return CA_OK; }   // resident clusters of the last cluster launch (0 before it)
     if (!std::strcmp(name, "diffusion_kernel")) {                             // 0 k_diffuse_sub, 1 k_diffuse_fused, 2 k_diffuse_slab, 3 k_diffuse_rows
         *value = !(c->fused && fused_supported(c->fplan)) ? 0 : (!c->fplan.tiled ? 1 : (c->fplan.rows ? 3 : 2));

@@ -605,6 +605,9 @@ struct FusedPlan {
     bool tiled = false;                // planes wider or taller than 64 sites: k_diffuse_slab
     int slab_warps = 0;
     bool rows = false;                 // k_diffuse_rows (ca_rows.cuh) covers this width; else k_diffuse_slab
+    int rows_rp = 1;                   // row pairs per lane of k_diffuse_rows on 96-wide planes (1: two rows; 2: four rows)
+    int slab_maxh = 0;                 // rows of the tallest slab
+    bool rp_attr_done[F_MAXNL + 1] = { false, false, false, false, false };
     int rows_cluster = 0;              // > 0: cluster variant of k_diffuse_rows with that many CTAs per plane
     int nclusters = 0;                 // clusters that can be resident at once (cudaOccupancyMaxActiveClusters)
     bool cluster_attr_done[F_MAXNL + 1] = { false, false, false, false, false };

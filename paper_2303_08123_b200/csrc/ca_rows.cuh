@@ -51,7 +51,7 @@ struct RowsCtx {
     uint32_t st_vote;              // byte offset (inside a state slot) of the 16 bytes of the warp's rows this lane votes on; ~0: none
     uint32_t in_slot, st_slot;     // bytes of one ring slot
     uint32_t ex_lvl;               // bytes of one level of the row exchange
-    u64 lamL, lamM, lamR;          // lambda pairs (row 0, row 1) for the lane's first / middle / last column; WALL and frozen rows folded in
+    u64 lamL[2], lamM[2], lamR[2]; // per row pair of the lane: lambda pairs (row 0, row 1) for its first / middle / last column; WALL and frozen rows folded in
     u64 zero2;
     uint32_t occ_nw;               // species 0: occupancy words of a plane this slab writes (else 0)
     // cluster variant: the CTA's first / last row pair also publishes its outer row into the neighbour CTA's exchange
@@ -76,18 +76,21 @@ __device__ __forceinline__ void cluster_barrier()
 }
 
 // CS = 1: y-slabs with a halo (any ny);  CS > 1: a thread-block cluster of CS CTAs holds ny = CS * hrows rows exactly, no halo
-template <int NL, int PX, int LRP, int CS = 1>
+// RP: row PAIRS per lane (1: two rows; 2: four rows -- half the row exchange per site, half the warps, twice the registers)
+template <int NL, int PX, int LRP, int CS = 1, int RP = 1>
 struct Rows {
     static constexpr int NX = PX * LRP;
-    static constexpr int RW = 32 / LRP;                                   // row pairs per warp
+    static constexpr int RW = 32 / LRP;                                   // row groups (of 2 * RP rows) per warp
+    static constexpr int PXR = PX * RP;                                   // packed registers per plane and level: [pair p][column k] at p * PX + k
     static constexpr uint32_t PITCH = (uint32_t)NX * 4u;
+    static_assert(CS == 1 || RP == 1, "the cluster variant is built for two rows per lane");
 
     static __device__ __forceinline__ RowsSeg *seg()
     {
         extern __shared__ __align__(128) unsigned char rsm_[];
         return reinterpret_cast<RowsSeg *>(rsm_ + F_SEG_OFF);
     }
-    static __device__ __forceinline__ u64 lam(const RowsCtx &c, int k) { return k == 0 ? c.lamL : (k == PX - 1 ? c.lamR : c.lamM); }
+    static __device__ __forceinline__ u64 lam(const RowsCtx &c, int p, int k) { return k == 0 ? c.lamL[p] : (k == PX - 1 ? c.lamR[p] : c.lamM[p]); }
 
     static __device__ __forceinline__ u64 shfl_up64(u64 v)
     {
@@ -104,22 +107,30 @@ struct Rows {
 
     // one sub-step of the diffusion part of [D S1] for this lane's PX x 2 points.  C = centre plane, M / P = planes z-1 / z+1,
     // up[k] / dn[k] = the row above / below the pair at column k.
-    static __device__ __forceinline__ void level(const u64 (&M)[PX], const u64 (&C)[PX], const u64 (&P)[PX], u64 (&N)[PX],
+    static __device__ __forceinline__ void level(const u64 (&M)[PXR], const u64 (&C)[PXR], const u64 (&P)[PXR], u64 (&N)[PXR],
                                                  const float (&up)[PX], const float (&dn)[PX], const RowsCtx &c)
     {
         const u64 six2 = pk(6.0f, 6.0f);
-        const u64 left = shfl_up64(C[PX - 1]);                               // column x0-1 (own value at the row's first lane: WALL side, lambda = 0)
-        const u64 right = shfl_down64(C[0]);                                 // column x0+PX
 #pragma unroll
-        for (int k = 0; k < PX; ++k) {
-            float c0, c1;
-            upk(C[k], c0, c1);
-            const u64 xs = add2(k == 0 ? left : C[k > 0 ? k - 1 : 0], k == PX - 1 ? right : C[k < PX - 1 ? k + 1 : 0]);   // xm + xp
-            const u64 ys = pk(__fadd_rn(up[k], c1), __fadd_rn(c0, dn[k]));   // ym + yp: row 0 has (up, row 1), row 1 has (row 0, dn)
-            const u64 zs = add2(M[k], P[k]);                                 // zm + zp
-            const u64 s6 = add2(add2(xs, ys), zs);
-            const u64 lap = sub2(s6, fma2(six2, C[k], c.zero2));             // 6*c rounded on its own (see Fused::level)
-            N[k] = fma2(lam(c, k), lap, C[k]);
+        for (int p = 0; p < RP; ++p) {
+            const u64 left = shfl_up64(C[p * PX + PX - 1]);                  // column x0-1 (own value at the row's first lane: WALL side, lambda = 0)
+            const u64 right = shfl_down64(C[p * PX]);                        // column x0+PX
+#pragma unroll
+            for (int k = 0; k < PX; ++k) {
+                const int e = p * PX + k;
+                float c0, c1;
+                upk(C[e], c0, c1);
+                // the row above the pair: the exchange for the lane's first pair, else row 1 of the pair above; likewise below
+                float ab = up[k], be = dn[k], t0, t1;
+                if (p > 0) { upk(C[(p > 0 ? p - 1 : 0) * PX + k], t0, t1); ab = t1; }
+                if (p < RP - 1) { upk(C[(p < RP - 1 ? p + 1 : 0) * PX + k], t0, t1); be = t0; }
+                const u64 xs = add2(k == 0 ? left : C[e > 0 ? e - 1 : 0], k == PX - 1 ? right : C[e < PXR - 1 ? e + 1 : 0]);   // xm + xp
+                const u64 ys = pk(__fadd_rn(ab, c1), __fadd_rn(c0, be));     // ym + yp: row 0 has (above, row 1), row 1 has (row 0, below)
+                const u64 zs = add2(M[e], P[e]);                             // zm + zp
+                const u64 s6 = add2(add2(xs, ys), zs);
+                const u64 lap = sub2(s6, fma2(six2, C[e], c.zero2));         // 6*c rounded on its own (see Fused::level)
+                N[e] = fma2(lam(c, p, k), lap, C[e]);
+            }
         }
     }
 
@@ -140,7 +151,7 @@ struct Rows {
 
     template <int PH, int K, bool STEADY, bool NOCELLS>
     static __device__ __forceinline__ void levels(const int t, const uint32_t q, const uint32_t exr, const uint32_t exw, const uint32_t outw,
-                                                  u64 (&h)[NL][3][PX], RowsCtx &c)
+                                                  u64 (&h)[NL][3][PXR], RowsCtx &c)
     {
         if constexpr (K <= NL) {
             // cluster variant: every row the neighbours need from this iteration is published once level NL-1 is done; the last
@@ -158,32 +169,46 @@ struct Rows {
 #pragma unroll
                 for (int k = 0; k < PX; ++k) {
                     up[k] = lds32f(eb + (uint32_t)k * 4u);                    // slab row row0 - 1
-                    dn[k] = lds32f(eb + 3u * PITCH + (uint32_t)k * 4u);       // slab row row0 + 2
+                    dn[k] = lds32f(eb + (uint32_t)(2 * RP + 1) * PITCH + (uint32_t)k * 4u);   // slab row row0 + 2 * RP
                 }
-                u64 nloc[PX];
-                u64 (&N)[PX] = *(K < NL ? &h[KO][sc] : &nloc);
+                u64 nloc[PXR];
+                u64 (&N)[PXR] = *(K < NL ? &h[KO][sc] : &nloc);
                 level(h[K - 1][sm], h[K - 1][sc], h[K - 1][sp], N, up, dn, c);
                 if (!NOCELLS && (((c.flags | c.slowmask) >> K) & 1u)) {      // cells in this warp's rows: source term and clamp
                     const uint32_t s = c.st_ring + ((q - (uint32_t)K) & (F_SRING - 1)) * c.st_slot + (c.lane_b >> 2);
 #pragma unroll
-                    for (int k = 0; k < PX; ++k) {
+                    for (int e = 0; e < PXR; ++e) {
+                        const uint32_t so = (uint32_t)(2 * (e / PX) * NX + e % PX);
                         uint32_t b0, b1;
-                        asm volatile("ld.shared.u8 %0, [%1];" : "=r"(b0) : "r"(s + (uint32_t)k));
-                        asm volatile("ld.shared.u8 %0, [%1];" : "=r"(b1) : "r"(s + (uint32_t)NX + (uint32_t)k));
-                        const u64 v = add2(N[k], pk(lds32f(c.lut + (b0 & 31u) * 4u), lds32f(c.lut + (b1 & 31u) * 4u)));
+                        asm volatile("ld.shared.u8 %0, [%1];" : "=r"(b0) : "r"(s + so));
+                        asm volatile("ld.shared.u8 %0, [%1];" : "=r"(b1) : "r"(s + so + (uint32_t)NX));
+                        const u64 v = add2(N[e], pk(lds32f(c.lut + (b0 & 31u) * 4u), lds32f(c.lut + (b1 & 31u) * 4u)));
                         float a, b;
                         upk(v, a, b);
-                        N[k] = pk(fmaxf(a, 0.0f), fmaxf(b, 0.0f));
+                        N[e] = pk(fmaxf(a, 0.0f), fmaxf(b, 0.0f));
                     }
                 }
-                // publish my two rows of level K: to the exchange for level K+1 of the next iteration, or (last level) to the staging slab
-                const uint32_t wb = K < NL ? exw + (uint32_t)K * c.ex_lvl + PITCH : outw;
+                // publish level K: my first and last row to the exchange for level K+1 of the next iteration (rows in between have
+                // their neighbours in this lane), or (last level) every row to the staging slab
+                if constexpr (K < NL) {
+                    const uint32_t wb = exw + (uint32_t)K * c.ex_lvl + PITCH;
 #pragma unroll
-                for (int k = 0; k < PX; ++k) {
-                    float a, b;
-                    upk(N[k], a, b);
-                    asm volatile("st.shared.f32 [%0], %1;" ::"r"(wb + (uint32_t)k * 4u), "f"(a) : "memory");
-                    asm volatile("st.shared.f32 [%0], %1;" ::"r"(wb + PITCH + (uint32_t)k * 4u), "f"(b) : "memory");
+                    for (int k = 0; k < PX; ++k) {
+                        float a, b, a2, b2;
+                        upk(N[k], a, b);
+                        upk(N[(RP - 1) * PX + k], a2, b2);
+                        asm volatile("st.shared.f32 [%0], %1;" ::"r"(wb + (uint32_t)k * 4u), "f"(a) : "memory");
+                        asm volatile("st.shared.f32 [%0], %1;" ::"r"(wb + (uint32_t)(2 * RP - 1) * PITCH + (uint32_t)k * 4u), "f"(b2) : "memory");
+                    }
+                } else {
+#pragma unroll
+                    for (int e = 0; e < PXR; ++e) {
+                        float a, b;
+                        upk(N[e], a, b);
+                        const uint32_t wo = outw + (uint32_t)(2 * (e / PX)) * PITCH + (uint32_t)(e % PX) * 4u;
+                        asm volatile("st.shared.f32 [%0], %1;" ::"r"(wo), "f"(a) : "memory");
+                        asm volatile("st.shared.f32 [%0], %1;" ::"r"(wo + PITCH), "f"(b) : "memory");
+                    }
                 }
                 if constexpr (CS > 1 && K < NL) {                            // my outer row is the neighbour CTA's halo row of level K
                     if (c.rem != 0u) {
@@ -200,14 +225,14 @@ struct Rows {
                 // WALL plane: every level equals the input there
                 const float *p = c.src + (size_t)zc * c.nxny;
 #pragma unroll
-                for (int k = 0; k < PX; ++k) h[KO][sc][k] = pk(p[k], p[NX + k]);
+                for (int e = 0; e < PXR; ++e) h[KO][sc][e] = pk(p[2 * (e / PX) * NX + e % PX], p[(2 * (e / PX) + 1) * NX + e % PX]);
             }
             levels<PH, K + 1, STEADY, NOCELLS>(t, q, exr, exw, outw, h, c);
         }
     }
 
     template <int PH, bool STEADY>
-    static __device__ __forceinline__ void step(const int i, u64 (&h)[NL][3][PX], RowsCtx &c)
+    static __device__ __forceinline__ void step(const int i, u64 (&h)[NL][3][PXR], RowsCtx &c)
     {
         // one body per phase: a second copy without the source-term code (as in k_diffuse_fused) costs more in instruction-cache
         // misses than the untaken branches it saves here (measured: 0.806 -> 0.775 ms at 64 x 96^3, 0.659 -> 0.608 ms at 96 x 80^3)
@@ -215,7 +240,7 @@ struct Rows {
     }
 
     template <int PH, bool STEADY, bool NOCELLS>
-    static __device__ __forceinline__ void step_body(const int i, u64 (&h)[NL][3][PX], RowsCtx &c)
+    static __device__ __forceinline__ void step_body(const int i, u64 (&h)[NL][3][PXR], RowsCtx &c)
     {
         const int t = c.t0 + i;
         const uint32_t q = c.itg + (uint32_t)i;
@@ -232,11 +257,12 @@ struct Rows {
         if (STEADY || (t >= c.ld_lo && t < c.ld_hi)) {
             const uint32_t a = c.in_ring + (uint32_t)PH * c.in_slot + c.lane_b;
 #pragma unroll
-            for (int k = 0; k < PX; ++k) {
-                const float v0 = lds32f(a + (uint32_t)k * 4u), v1 = lds32f(a + PITCH + (uint32_t)k * 4u);
-                h[0][PH][k] = pk(v0, v1);
-                asm volatile("st.shared.f32 [%0], %1;" ::"r"(exw + PITCH + (uint32_t)k * 4u), "f"(v0) : "memory");
-                asm volatile("st.shared.f32 [%0], %1;" ::"r"(exw + 2u * PITCH + (uint32_t)k * 4u), "f"(v1) : "memory");
+            for (int e = 0; e < PXR; ++e) {
+                const int pp = e / PX, k = e % PX;
+                const float v0 = lds32f(a + (uint32_t)(2 * pp) * PITCH + (uint32_t)k * 4u), v1 = lds32f(a + (uint32_t)(2 * pp + 1) * PITCH + (uint32_t)k * 4u);
+                h[0][PH][e] = pk(v0, v1);
+                if (pp == 0) asm volatile("st.shared.f32 [%0], %1;" ::"r"(exw + PITCH + (uint32_t)k * 4u), "f"(v0) : "memory");
+                if (pp == RP - 1) asm volatile("st.shared.f32 [%0], %1;" ::"r"(exw + (uint32_t)(2 * RP) * PITCH + (uint32_t)k * 4u), "f"(v1) : "memory");
                 if constexpr (CS > 1) {
                     if (c.rem != 0u) st_cluster_f32(c.rem + (exw - c.ex_lane) + (uint32_t)k * 4u, c.rem_row1 ? v1 : v0);
                 }
@@ -279,10 +305,10 @@ struct Rows {
 };
 
 // grid: persistent, one CTA per SM; block = Gm.nwarps warps
-template <int NL, int PX, int LRP, int MAXW, int CS>
+template <int NL, int PX, int LRP, int MAXW, int CS, int RP>
 __global__ void __launch_bounds__(MAXW * 32, 1) k_diffuse_rows(const FusedArgs A, const RowsGeom Gm)
 {
-    typedef Rows<NL, PX, LRP, CS> R;
+    typedef Rows<NL, PX, LRP, CS, RP> R;
     extern __shared__ __align__(128) unsigned char rsm[];
     constexpr int NX = PX * LRP, RW = 32 / LRP;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -321,13 +347,13 @@ __global__ void __launch_bounds__(MAXW * 32, 1) k_diffuse_rows(const FusedArgs A
     const int wid = CS > 1 ? (int)blockIdx.x / CS : (int)blockIdx.x;       // the CTAs of a cluster work through the same segments in lockstep
     long long p = Gm.start[wid];
     const long long p_end = Gm.start[wid + 1];
-    u64 h[NL][3][PX];
+    u64 h[NL][3][PX * RP];
 #pragma unroll
     for (int k = 0; k < NL; ++k)
 #pragma unroll
         for (int s = 0; s < 3; ++s)
 #pragma unroll
-            for (int j = 0; j < PX; ++j) h[k][s][j] = 0ull;
+            for (int j = 0; j < PX * RP; ++j) h[k][s][j] = 0ull;
 
     while (p < p_end) {
         const int unit = (int)(p / nzi);
@@ -337,15 +363,15 @@ __global__ void __launch_bounds__(MAXW * 32, 1) k_diffuse_rows(const FusedArgs A
         c.zb = (int)min((long long)(A.nz - 1), (long long)c.za + (p_end - p));
         p += c.zb - c.za;
         const int ty0 = A.sy0[slab], ty1 = A.sy1[slab], oy0 = A.so0[slab], oy1 = A.so1[slab];
-        const int rows = ty1 - ty0;                                            // even, >= 2 * RW
-        const int row0 = 2 * min(gl, rows / 2 - 1);                            // pairs beyond a short slab: duplicates of its last pair (same values to the same addresses)
+        const int rows = ty1 - ty0;                                            // a multiple of 2 * RP, >= 2 * RP * RW
+        const int row0 = 2 * RP * min(gl, rows / (2 * RP) - 1);                // groups beyond a short slab: duplicates of its last group (same values to the same addresses)
         const size_t ubase = (size_t)b * (size_t)c.nxny * (size_t)A.nz;
         c.lane_b = (uint32_t)(row0 * NX + x0) * 4u;
         c.ex_lane = base + Gm.off_ex + c.lane_b;
         c.src = A.src[sp] + ubase + (size_t)(ty0 + row0) * NX + x0;
-        {   // vote bytes: the warp's 2 * RW rows (clamped into the slab), 16 bytes per lane
-            const int vr0 = min(2 * RW * warp, rows - 2 * RW);
-            c.st_vote = lane < (2 * RW * NX) / 16 ? (uint32_t)(vr0 * NX + 16 * lane) : 0xFFFFFFFFu;
+        {   // vote bytes: the warp's 2 * RP * RW rows (clamped into the slab), 16 bytes per lane
+            const int vr0 = min(2 * RP * RW * warp, rows - 2 * RP * RW);
+            c.st_vote = lane < (2 * RP * RW * NX) / 16 ? (uint32_t)(vr0 * NX + 16 * lane) : 0xFFFFFFFFu;
         }
         c.t0 = c.za - NL;
         c.nsteps = c.zb - c.za + 2 * NL;
@@ -358,11 +384,15 @@ __global__ void __launch_bounds__(MAXW * 32, 1) k_diffuse_rows(const FusedArgs A
         {
             const float l = A.lam[sp];
             // the slab's first / last row is frozen (WALL, or halo edge); in a cluster only the lattice's own first / last row (WALL)
-            const float m0 = (CS > 1 ? ty0 + row0 > 0 : row0 > 0) ? 1.0f : 0.0f;
-            const float m1 = (CS > 1 ? ty0 + row0 + 1 < A.ny - 1 : row0 + 1 < rows - 1) ? 1.0f : 0.0f;
-            c.lamM = pk(l * m0, l * m1);
-            c.lamL = lx == 0 ? pk(0.0f, 0.0f) : c.lamM;                        // x = 0 and x = nx-1 are WALL
-            c.lamR = lx == LRP - 1 ? pk(0.0f, 0.0f) : c.lamM;
+#pragma unroll
+            for (int pp = 0; pp < RP; ++pp) {
+                const int r0 = row0 + 2 * pp;
+                const float m0 = (CS > 1 ? ty0 + r0 > 0 : r0 > 0) ? 1.0f : 0.0f;
+                const float m1 = (CS > 1 ? ty0 + r0 + 1 < A.ny - 1 : r0 + 1 < rows - 1) ? 1.0f : 0.0f;
+                c.lamM[pp] = pk(l * m0, l * m1);
+                c.lamL[pp] = lx == 0 ? pk(0.0f, 0.0f) : c.lamM[pp];            // x = 0 and x = nx-1 are WALL
+                c.lamR[pp] = lx == LRP - 1 ? pk(0.0f, 0.0f) : c.lamM[pp];
+            }
         }
         if (tid == 0) {                                                        // every reader of the old values is past the last barrier of the previous segment
             RowsSeg *sg = R::seg();
@@ -419,21 +449,22 @@ inline bool rows_shape(int nx, int &px, int &lrp, int &maxw)
     return false;
 }
 
-template <int NL, int PX, int LRP, int MAXW>
+template <int NL, int PX, int LRP, int MAXW, int RP>
 inline cudaError_t rows_launch_t(FusedPlan &F, const FusedArgs &A, int grid, cudaStream_t st)
 {
     RowsGeom G{};
     rows_smem(A.nx, NL, A.rga, G);
-    G.nwarps = F.slab_warps;
+    G.nwarps = RP == 1 ? F.slab_warps : (F.slab_maxh / (2 * RP) + 32 / LRP - 1) / (32 / LRP);
     const int units = A.batch * 3 * A.nslab;
     if (grid > F_MAXGRID) grid = F_MAXGRID;
     fused_split_cached(F, units, A.nz - 2, NL, grid, G.start);
-    if (!F.attr_done[NL]) {
-        cudaError_t e = cudaFuncSetAttribute(k_diffuse_rows<NL, PX, LRP, MAXW, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    bool &done = RP == 1 ? F.attr_done[NL] : F.rp_attr_done[NL];
+    if (!done) {
+        cudaError_t e = cudaFuncSetAttribute(k_diffuse_rows<NL, PX, LRP, MAXW, 1, RP>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         if (e != cudaSuccess) return e;
-        F.attr_done[NL] = true;
+        done = true;
     }
-    k_diffuse_rows<NL, PX, LRP, MAXW, 1><<<grid, G.nwarps * 32, G.smem_bytes, st>>>(A, G);
+    k_diffuse_rows<NL, PX, LRP, MAXW, 1, RP><<<grid, G.nwarps * 32, G.smem_bytes, st>>>(A, G);
     return cudaGetLastError();
 }
 
@@ -449,7 +480,7 @@ inline cudaError_t rows_launch_cluster_t(FusedPlan &F, const FusedArgs &A0, cuda
     RowsGeom G{};
     rows_smem(A.nx, NL, hrows, G);
     G.nwarps = (hrows / 2) / (32 / LRP);
-    auto kern = k_diffuse_rows<NL, PX, LRP, MAXW, CS>;
+    auto kern = k_diffuse_rows<NL, PX, LRP, MAXW, CS, 1>;
     cudaLaunchConfig_t cfg = {};
     cfg.blockDim = dim3((unsigned int)(G.nwarps * 32));
     cfg.dynamicSmemBytes = G.smem_bytes;
@@ -482,8 +513,9 @@ template <int NL>
 inline cudaError_t rows_launch(FusedPlan &F, const FusedArgs &A, int grid, cudaStream_t st)
 {
     if (A.nx == 96 && F.rows_cluster == 3) return rows_launch_cluster_t<NL, 3, 32, 16, 3>(F, A, st);   // BASELINE configs[2]: 3 CTAs x 32 rows
-    if (A.nx == 96) return rows_launch_t<NL, 3, 32, 16>(F, A, grid, st);      // 96-wide planes of any height: slabs with a halo
-    return rows_launch_t<NL, 5, 16, 12>(F, A, grid, st);                      // BASELINE configs[3]
+    if (A.nx == 96 && F.rows_rp == 2) return rows_launch_t<NL, 3, 32, 8, 2>(F, A, grid, st);   // four rows per lane: 8 warps, up to 255 registers
+    if (A.nx == 96) return rows_launch_t<NL, 3, 32, 16, 1>(F, A, grid, st);   // 96-wide planes of any height: slabs with a halo
+    return rows_launch_t<NL, 5, 16, 12, 1>(F, A, grid, st);                   // BASELINE configs[3]
 }
 
 // Does the rows kernel cover this lattice?  Fills the slab table of F.args (rga = rows a CTA holds).
@@ -498,6 +530,7 @@ inline bool rows_configure(const KParams &P, FusedPlan &F)
     for (int t = 0; t < F.args.nslab; ++t) maxh = std::max(maxh, F.args.sy1[t] - F.args.sy0[t]);
     F.args.rga = hrows;
     F.slab_warps = (maxh / 2 + rw - 1) / rw;
+    F.slab_maxh = maxh;
     RowsGeom G{};
     if (rows_smem(P.nx, F_MAXNL, hrows, G) > 227 * 1024) return false;
     F.lrp = lrp;

@@ -169,3 +169,49 @@ def test_get_option_reports_the_diffusion_kernel_that_serves_a_lattice():
     with pytest.raises(binding.CaError):
         g.set_option("rows_cluster", 3)              # clusters of 3 exist for 96 x 96 planes only
     g.close()
+
+
+def test_two_contexts_driven_by_two_host_threads_agree_with_serial_runs():
+    """kernel attributes and the work-split cache used to be process-wide statics; ctypes releases the GIL, so two
+    host threads can drive two contexts at once.  Two contexts with DIFFERENT lattices (different diffusion kernels, different
+    split tables) stepped concurrently must end exactly where the same contexts end when stepped one after the other."""
+    import threading
+    p = w.stress_params()
+    specs = [((64, 64, 10), 11), ((96, 96, 8), 12), ((32, 32, 12), 13)]
+
+    def make(dims, seed):
+        g = binding.CaBatch(3, *dims, p, max_frac=2)
+        g.set_option("graph_steps", 4)
+        g.seed("ball", radius=3.0, rng_seed=seed, sim_id_base=1)
+        g.set_protocols(np.full((3, 1), 3.0), np.full((3, 1), 0.02))
+        return g
+
+    serial = []
+    for dims, seed in specs:
+        g = make(dims, seed)
+        g.step(48)
+        serial.append([g.get_state(b) for b in range(3)])
+        g.close()
+    ctxs = [make(dims, seed) for dims, seed in specs]
+    errs = []
+
+    def drive(g):
+        try:
+            for _ in range(12):
+                g.step(4)
+            g.sync()
+        except Exception as e:                                   # noqa: BLE001
+            errs.append(e)
+
+    ts = [threading.Thread(target=drive, args=(g,)) for g in ctxs]
+    for t in ts:
+        t.start()
+    for t in ts:
+        t.join()
+    assert not errs, errs
+    for g, ref in zip(ctxs, serial):
+        for b in range(3):
+            out = g.get_state(b)
+            for k in ("state", "clock", "damage", "o2", "glc", "h"):
+                assert np.array_equal(out[k], ref[b][k]), (g.nx, b, k)
+        g.close()
