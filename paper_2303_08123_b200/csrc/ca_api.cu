@@ -673,7 +673,7 @@ int ca_set_option(ca_ctx *c, const char *name, int value)
     }
     if (!std::strcmp(name, "rows_cluster")) {                                  // 0: k_diffuse_rows on slabs with a halo; 3: cluster of 3 CTAs per 96 x 96 plane
         if (!(value == 0 || (value == 3 && c->P.nx == 96 && c->P.ny == 96 && c->fplan.rows))) return fail(c, CA_EINVAL, "rows_cluster must be 0, or 3 on 96 x 96 planes");
-        c->fplan.rows_cluster = value; drop_graphs(c); return CA_OK;
+        c->fplan.rows_cluster = value; drop_graphs(c); return CA_OK;          // the cluster variant is built for two rows per lane: it ignores rows_rp
     }
     if (!std::strcmp(name, "cluster")) {
         if (value != 1 && value != 2 && value != 4 && value != 8) return fail(c, CA_EINVAL, "cluster must be 1, 2, 4 or 8");

@@ -2,7 +2,8 @@
 // 96^3, 80^3): NL (<= 4) sub-steps of [D S1] in ONE pass over HBM, like k_diffuse_fused, with a lane layout that covers a
 // WHOLE lattice row of width nx = PX * LRP without seams:
 //
-//   * a lane owns PX consecutive sites (PX = 3 for 96 = 3 * 32 lanes, PX = 5 for 80 = 5 * 16 lanes) of TWO rows; the packed
+//   * a lane owns PX consecutive sites (PX = 3 for 96 = 3 * 32 lanes, PX = 5 for 80 = 5 * 16 lanes) of TWO rows (RP = 1) or of
+//     FOUR rows (RP = 2: two packed row pairs; the default on 96-wide planes: half the row exchange per site, 8 warps); the packed
 //     f32x2 registers pair the two ROWS of one column, so x-neighbours inside a lane are whole registers (one packed add),
 //     only the lane's first / last column needs the neighbour lane (two 64-bit shuffles per level), and odd PX is fine;
 //   * a CTA holds a y-slab of whole rows (32 rows for 96-wide planes, 44 for 80): contiguous in memory, so a slab of a field
@@ -538,6 +539,9 @@ inline bool rows_configure(const KParams &P, FusedPlan &F)
     // OFF by default: measured 0.851 ms against 0.769 ms for the slabs with a halo at 64 x 96^3 (45 clusters = 135 of 148 SMs
     // resident, and an iteration of three SMs in lockstep costs 4075 cycles against 3063), DESIGN.md section 7.
     F.rows_cluster = 0;
+    // four rows per lane on 96-wide planes (8 warps, 240 registers): 5.58 against 5.70 ms per launch at 512 x 96^3; the lane
+    // layout of 80-wide planes (5 sites per lane) would need more than 255 registers for it
+    F.rows_rp = P.nx == 96 ? 2 : 1;
     return true;
 }
 

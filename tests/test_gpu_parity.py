@@ -227,9 +227,9 @@ def test_state_roundtrip_broadcast_and_errors():
     ((32, 32, 12), 5, {"graph_steps": 2}),                   # 3 + 2: odd number of flips per step
     ((48, 32, 9), 2, {}),                                    # run-time-dims fused kernel, map built by k_occ_map
     ((96, 96, 9), 4, {}),                                    # configs[2] plane: k_diffuse_rows, 4 y-slabs of 32 rows, spheroid on the cuts
-    ((96, 96, 9), 4, {"rows_cluster": 3, "graph_steps": 4}), # the same plane on clusters of 3 CTAs: boundary rows through distributed shared memory
-    ((96, 96, 9), 4, {"rows_rp": 2}),                        # the same plane with four rows per lane (8 warps)
-    ((96, 40, 7), 3, {"rows_rp": 2, "graph_steps": 2}),      # ... on a non-square plane with a short last slab, 3 levels
+    ((96, 96, 9), 4, {"rows_rp": 1, "rows_cluster": 3, "graph_steps": 4}), # the same plane on clusters of 3 CTAs: boundary rows through distributed shared memory
+    ((96, 96, 9), 4, {"rows_rp": 1}),                        # the same plane with two rows per lane (16 warps; four rows per lane is the default)
+    ((96, 40, 7), 3, {"rows_rp": 1, "graph_steps": 2}),      # ... on a non-square plane with a short last slab, 3 levels
     ((80, 80, 9), 4, {"graph_steps": 6}),                    # configs[3] plane: k_diffuse_rows, 2 y-slabs of 44 rows
     ((96, 40, 7), 4, {}),                                    # k_diffuse_rows on a plane that is not square: 2 slabs, map from k_occ_map
     ((80, 52, 6), 2, {}),                                    # k_diffuse_rows, 2 levels, a short second slab (duplicate row pairs)
