@@ -84,6 +84,12 @@ struct Rows {
     static constexpr int RW = 32 / LRP;                                   // row groups (of 2 * RP rows) per warp
     static constexpr int PXR = PX * RP;                                   // packed registers per plane and level: [pair p][column k] at p * PX + k
     static constexpr uint32_t PITCH = (uint32_t)NX * 4u;
+    // Row pitch of the EXCHANGE buffer.  A warp with two row groups (LRP = 16) has its half-warps 2 * RP rows apart; at the
+    // lattice pitch of 80 words that is a multiple of 32 banks, so lanes l and l + 16 collide on every exchange access (ncu on
+    // 96 x 80^3: shared pipe 68 %, short_scoreboard and mio_throttle the top stalls).  88 words put the second half-warp 16
+    // banks further: with the lane stride of 5 words the 32 lanes then hit 32 different banks.  The input ring and the staging
+    // slab are moved by bulk copies at the lattice pitch and cannot be padded.
+    static constexpr uint32_t EXP = (RW > 1 && ((uint32_t)(2 * RP * NX) % 32u) == 0u) ? PITCH + 32u : PITCH;
     static_assert(CS == 1 || RP == 1, "the cluster variant is built for two rows per lane");
 
     static __device__ __forceinline__ RowsSeg *seg()
@@ -170,7 +176,7 @@ struct Rows {
 #pragma unroll
                 for (int k = 0; k < PX; ++k) {
                     up[k] = lds32f(eb + (uint32_t)k * 4u);                    // slab row row0 - 1
-                    dn[k] = lds32f(eb + (uint32_t)(2 * RP + 1) * PITCH + (uint32_t)k * 4u);   // slab row row0 + 2 * RP
+                    dn[k] = lds32f(eb + (uint32_t)(2 * RP + 1) * EXP + (uint32_t)k * 4u);     // slab row row0 + 2 * RP
                 }
                 u64 nloc[PXR];
                 u64 (&N)[PXR] = *(K < NL ? &h[KO][sc] : &nloc);
@@ -192,14 +198,14 @@ struct Rows {
                 // publish level K: my first and last row to the exchange for level K+1 of the next iteration (rows in between have
                 // their neighbours in this lane), or (last level) every row to the staging slab
                 if constexpr (K < NL) {
-                    const uint32_t wb = exw + (uint32_t)K * c.ex_lvl + PITCH;
+                    const uint32_t wb = exw + (uint32_t)K * c.ex_lvl + EXP;
 #pragma unroll
                     for (int k = 0; k < PX; ++k) {
                         float a, b, a2, b2;
                         upk(N[k], a, b);
                         upk(N[(RP - 1) * PX + k], a2, b2);
                         asm volatile("st.shared.f32 [%0], %1;" ::"r"(wb + (uint32_t)k * 4u), "f"(a) : "memory");
-                        asm volatile("st.shared.f32 [%0], %1;" ::"r"(wb + (uint32_t)(2 * RP - 1) * PITCH + (uint32_t)k * 4u), "f"(b2) : "memory");
+                        asm volatile("st.shared.f32 [%0], %1;" ::"r"(wb + (uint32_t)(2 * RP - 1) * EXP + (uint32_t)k * 4u), "f"(b2) : "memory");
                     }
                 } else {
 #pragma unroll
@@ -262,8 +268,8 @@ struct Rows {
                 const int pp = e / PX, k = e % PX;
                 const float v0 = lds32f(a + (uint32_t)(2 * pp) * PITCH + (uint32_t)k * 4u), v1 = lds32f(a + (uint32_t)(2 * pp + 1) * PITCH + (uint32_t)k * 4u);
                 h[0][PH][e] = pk(v0, v1);
-                if (pp == 0) asm volatile("st.shared.f32 [%0], %1;" ::"r"(exw + PITCH + (uint32_t)k * 4u), "f"(v0) : "memory");
-                if (pp == RP - 1) asm volatile("st.shared.f32 [%0], %1;" ::"r"(exw + (uint32_t)(2 * RP) * PITCH + (uint32_t)k * 4u), "f"(v1) : "memory");
+                if (pp == 0) asm volatile("st.shared.f32 [%0], %1;" ::"r"(exw + EXP + (uint32_t)k * 4u), "f"(v0) : "memory");
+                if (pp == RP - 1) asm volatile("st.shared.f32 [%0], %1;" ::"r"(exw + (uint32_t)(2 * RP) * EXP + (uint32_t)k * 4u), "f"(v1) : "memory");
                 if constexpr (CS > 1) {
                     if (c.rem != 0u) st_cluster_f32(c.rem + (exw - c.ex_lane) + (uint32_t)k * 4u, c.rem_row1 ? v1 : v0);
                 }
@@ -321,7 +327,7 @@ __global__ void __launch_bounds__(MAXW * 32, 1) k_diffuse_rows(const FusedArgs A
     c.nxny = NX * A.ny; c.nz = A.nz;
     c.bars = base; c.in_ring = base + Gm.off_in; c.st_ring = base + Gm.off_st; c.out_ring = base + Gm.off_out;
     c.in_slot = (uint32_t)(Gm.hrows * NX) * 4u; c.st_slot = (uint32_t)(Gm.hrows * NX);
-    c.ex_lvl = (uint32_t)(Gm.hrows + 2) * R::PITCH;
+    c.ex_lvl = (uint32_t)(Gm.hrows + 2) * R::EXP;
     c.itg = 0; c.par = 0;
     c.zero2 = pk(A.zero, A.zero);
     if (tid == 0) {
@@ -336,7 +342,7 @@ __global__ void __launch_bounds__(MAXW * 32, 1) k_diffuse_rows(const FusedArgs A
     if constexpr (CS > 1) {
         // the CTAs of a cluster hold consecutive ranges of hrows rows; exchange row 0 / hrows + 1 of a CTA is written by its neighbour
         const int pairs = Gm.hrows / 2;
-        if (gl == 0 && rank > 0) c.rem = map_to_rank(base + Gm.off_ex + (uint32_t)(Gm.hrows + 1) * R::PITCH + (uint32_t)x0 * 4u, (uint32_t)(rank - 1));
+        if (gl == 0 && rank > 0) c.rem = map_to_rank(base + Gm.off_ex + (uint32_t)(Gm.hrows + 1) * R::EXP + (uint32_t)x0 * 4u, (uint32_t)(rank - 1));
         if (gl == pairs - 1 && rank < CS - 1) { c.rem = map_to_rank(base + Gm.off_ex + (uint32_t)x0 * 4u, (uint32_t)(rank + 1)); c.rem_row1 = true; }
         cluster_barrier();                                                   // nobody writes into an exchange that is still being zeroed
         cluster_arrive();                                                    // pairs with the wait at the top of the first iteration
@@ -368,7 +374,7 @@ __global__ void __launch_bounds__(MAXW * 32, 1) k_diffuse_rows(const FusedArgs A
         const int row0 = 2 * RP * min(gl, rows / (2 * RP) - 1);                // groups beyond a short slab: duplicates of its last group (same values to the same addresses)
         const size_t ubase = (size_t)b * (size_t)c.nxny * (size_t)A.nz;
         c.lane_b = (uint32_t)(row0 * NX + x0) * 4u;
-        c.ex_lane = base + Gm.off_ex + c.lane_b;
+        c.ex_lane = base + Gm.off_ex + (uint32_t)row0 * R::EXP + (uint32_t)x0 * 4u;
         c.src = A.src[sp] + ubase + (size_t)(ty0 + row0) * NX + x0;
         {   // vote bytes: the warp's 2 * RP * RW rows (clamped into the slab), 16 bytes per lane
             const int vr0 = min(2 * RP * RW * warp, rows - 2 * RP * RW);
@@ -429,14 +435,16 @@ __global__ void __launch_bounds__(MAXW * 32, 1) k_diffuse_rows(const FusedArgs A
 }
 
 // ------------------------------------------------------------------ host side --
-inline size_t rows_smem(int nx, int nl, int hrows, RowsGeom &G)
+// expitch_words: row pitch of the exchange buffer in words (Rows::EXP / 4)
+inline size_t rows_smem(int nx, int nl, int hrows, RowsGeom &G, int expitch_words = 0)
 {
+    const int exw = expitch_words ? expitch_words : nx;
     size_t o = 128;
     G.hrows = hrows;
     G.off_lut = (uint32_t)o; o += 96 * 4; o = (o + 127) / 128 * 128;
     G.off_in = (uint32_t)o; o += (size_t)F_RING * hrows * nx * 4; o = (o + 127) / 128 * 128;
     G.off_st = (uint32_t)o; o += (size_t)F_SRING * hrows * nx; o = (o + 127) / 128 * 128;
-    G.off_ex = (uint32_t)o; o += (size_t)2 * nl * (hrows + 2) * nx * 4; o = (o + 127) / 128 * 128;
+    G.off_ex = (uint32_t)o; o += (size_t)2 * nl * (hrows + 2) * exw * 4; o = (o + 127) / 128 * 128;
     G.off_out = (uint32_t)o; o += (size_t)2 * hrows * nx * 4; o = (o + 127) / 128 * 128;
     G.smem_bytes = (uint32_t)o;
     return o;
@@ -454,7 +462,7 @@ template <int NL, int PX, int LRP, int MAXW, int RP>
 inline cudaError_t rows_launch_t(FusedPlan &F, const FusedArgs &A, int grid, cudaStream_t st)
 {
     RowsGeom G{};
-    rows_smem(A.nx, NL, A.rga, G);
+    rows_smem(A.nx, NL, A.rga, G, (int)(Rows<NL, PX, LRP, 1, RP>::EXP / 4u));
     G.nwarps = RP == 1 ? F.slab_warps : (F.slab_maxh / (2 * RP) + 32 / LRP - 1) / (32 / LRP);
     const int units = A.batch * 3 * A.nslab;
     if (grid > F_MAXGRID) grid = F_MAXGRID;
@@ -533,7 +541,8 @@ inline bool rows_configure(const KParams &P, FusedPlan &F)
     F.slab_warps = (maxh / 2 + rw - 1) / rw;
     F.slab_maxh = maxh;
     RowsGeom G{};
-    if (rows_smem(P.nx, F_MAXNL, hrows, G) > 227 * 1024) return false;
+    const int exw = (rw > 1 && (2 * P.nx) % 32 == 0) ? P.nx + 8 : P.nx;        // Rows::EXP for two rows per lane (the largest exchange)
+    if (rows_smem(P.nx, F_MAXNL, hrows, G, exw) > 227 * 1024) return false;
     F.lrp = lrp;
     // The cluster variant (96 rows = 3 CTAs x 16 warps x one row pair, no halo) is correct and selectable ("rows_cluster" = 3) but
     // OFF by default: measured 0.851 ms against 0.769 ms for the slabs with a halo at 64 x 96^3 (45 clusters = 135 of 148 SMs
