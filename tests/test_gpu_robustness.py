@@ -166,8 +166,21 @@ def test_get_option_reports_the_diffusion_kernel_that_serves_a_lattice():
         g.get_option("no_such_option")
     g.close()
     g = binding.CaBatch(1, 80, 80, 8, p)
+    assert g.get_option("rows_rp") == 1              # 5 sites per lane: four rows per lane would need more than 255 registers
     with pytest.raises(binding.CaError):
         g.set_option("rows_cluster", 3)              # clusters of 3 exist for 96 x 96 planes only
+    with pytest.raises(binding.CaError):
+        g.set_option("rows_rp", 2)                   # ... and four rows per lane for 96-wide planes only
+    g.close()
+    g = binding.CaBatch(1, 96, 40, 8, p)
+    assert g.get_option("rows_rp") == 2              # the default on 96-wide planes
+    g.set_option("rows_rp", 1)
+    assert g.get_option("rows_rp") == 1
+    with pytest.raises(binding.CaError):
+        g.set_option("rows_rp", 3)
+    g.close()
+    g = binding.CaBatch(1, 64, 64, 8, p)
+    assert g.get_option("rows_rp") == 0              # not a k_diffuse_rows lattice
     g.close()
 
 
