@@ -401,7 +401,13 @@ __global__ void __launch_bounds__(MAXW * 32, 1) k_diffuse_rows(const FusedArgs A
                 c.lamR[pp] = lx == LRP - 1 ? pk(0.0f, 0.0f) : c.lamM[pp];
             }
         }
-        if (tid == 0) {                                                        // every reader of the old values is past the last barrier of the previous segment
+        // The store of the previous segment's last plane is issued by thread 32 AFTER that segment's last barrier, from the descriptor
+        // below (dst_rows, out_off, out_bytes).  Without this barrier thread 0 can overwrite the descriptor first, and the plane goes
+        // to the NEXT segment's destination -- another slab, species or simulation.  (Round 2 had that race for a few commits after
+        // the stores moved from thread 0 to thread 32: rare, invisible in 60-step parity windows, found when two identical runs of the
+        // configs[3] job at batch 512 disagreed; tests/test_gpu_long.py::test_full_batch_runs_are_deterministic_... guards it.)
+        __syncthreads();
+        if (tid == 0) {
             RowsSeg *sg = R::seg();
             sg->src_rows = A.src[sp] + ubase + (size_t)ty0 * NX;
             sg->st_rows = A.state + ubase + (size_t)ty0 * NX;

@@ -159,3 +159,45 @@ def test_c5_sized_batch_4096_sims():
         assert_fields_bitwise(gs, r.get_state(), "sim %d" % b)
         assert fit[b] == r.fitness()
     g.close()
+
+
+@pytest.mark.parametrize("k,batch", [(4, 512), (3, 192)])
+def test_full_batch_runs_are_deterministic_and_match_the_generic_path(k, batch):
+    """Two identical fast-path contexts and one fully generic one (per-sub-step diffusion, scan kernels) of the configs[3] /
+    configs[2] job at a batch with thousands of work units per diffusion launch, 1800 CA steps from the saved tumour: every
+    count of every simulation must agree, and the complete state of a few simulations bit for bit.  Regression test for a
+    race in k_diffuse_rows (the bulk store of a segment's last plane read its descriptor after the next segment's had been
+    written): about one simulation in 500 was corrupted within 1200 steps, which no 60-step parity window ever saw."""
+    p = w.default_params()
+    cfg = w.config(k)
+    dims = cfg["dims"]
+    one = binding.CaBatch(1, *dims, p, max_frac=1)
+    one.seed("ball", center=tuple(d // 2 for d in dims), radius=9.0, rng_seed=cfg["rng_seed"], shared_init=True)
+    one.step(600)
+    snap = one.get_state(0)
+    one.close()
+    res, ctxs = [], []
+    for opts in ({}, {}, {"fused": 0, "cell_path": 0}):
+        g = binding.CaBatch(batch, *dims, p, max_frac=cfg["dose"].shape[1])
+        for name, v in opts.items():
+            g.set_option(name, v)
+        g.set_state(0, batch, state=snap["state"], clock=snap["clock"], damage=snap["damage"], o2=snap["o2"], glc=snap["glc"], h=snap["h"], step=snap["step"])
+        g.set_rng(cfg["rng_seed"], 0)
+        dose = cfg["dose"][:batch].copy(); delay = cfg["delay"][:batch].copy()
+        delay[:, 0] = 1.0 + (np.arange(batch) % 3) * 0.5          # first fractions inside the window, at three different steps
+        g.set_protocols(dose, delay, cfg["nfrac"][:batch], t0_h=1.0)
+        g.step(1800)
+        res.append(g.counts())
+        ctxs.append(g)
+    assert res[0][:, 1].min() > 0                                  # every simulation was irradiated
+    for i in (1, 2):
+        bad = np.argwhere((res[i] != res[0]).any(axis=1)).ravel()
+        assert len(bad) == 0, (i, bad[:8].tolist(), res[i][bad[0]].tolist(), res[0][bad[0]].tolist())
+    for b in (0, batch // 3, batch - 1):
+        ref = ctxs[2].get_state(b)
+        for g in ctxs[:2]:
+            out = g.get_state(b)
+            for name in ("state", "clock", "damage", "o2", "glc", "h"):
+                assert np.array_equal(out[name], ref[name]), (b, name)
+    for g in ctxs:
+        g.close()
