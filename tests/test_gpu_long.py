@@ -161,7 +161,7 @@ def test_c5_sized_batch_4096_sims():
     g.close()
 
 
-@pytest.mark.parametrize("k,batch", [(4, 512), (3, 192)])
+@pytest.mark.parametrize("k,batch", [(4, 512), (3, 512)])
 def test_full_batch_runs_are_deterministic_and_match_the_generic_path(k, batch):
     """Two identical fast-path contexts and one fully generic one (per-sub-step diffusion, scan kernels) of the configs[3] /
     configs[2] job at a batch with thousands of work units per diffusion launch, 1800 CA steps from the saved tumour: every
